@@ -1,0 +1,128 @@
+"""Pins for oracle tier 2 (plain block-sparse DMRG) against tier 1 (brute-force FCI) and invariants.
+DESIGN.md C5: H_eff x vs P^T H P x at every bond; untruncated sweeps vs FCI energy and RDMs; RDM invariants."""
+import numpy as np
+import pytest
+
+from oracle import fci, dmrg
+from synth import random_dense, random_mps, make_config
+
+
+@pytest.mark.parametrize("k,n,s2,D", [(4, 4, 0, 8), (5, 5, 1, 10), (6, 8, 0, 12), (6, 3, -1, 12)])
+def test_heff_vs_bruteforce_every_bond(k, n, s2, D):
+    h, eri = random_dense(k, 40 + k)
+    ham = dmrg.Ham(h, eri)
+    sp = fci.FCISpace(k, n, s2)
+    for i in range(k - 1):
+        mps = random_mps(k, n, s2, D, seed=70 + i, gauge="LR:%d" % i)
+        L = dmrg.build_left(mps, ham, i)[-1]
+        R = dmrg.build_right(mps, ham, i + 2)[i + 2]
+        for side in ("L", "R"):
+            H = dmrg.Heff(L, R, ham, i, normal_side=side)
+            lay, nnz = fci.heff_layout(mps, i)
+            assert nnz == H.nnz and [tuple(b) for b in lay] == [tuple(b) for b in H.layout]
+            x = np.random.default_rng(i).normal(size=nnz)
+            y = H.apply(x)
+            yb = fci.heff_apply_bruteforce(mps, i, h, eri, x, sp)
+            assert np.linalg.norm(y - yb) <= 1e-13 * np.linalg.norm(yb)
+
+
+def test_heff_symmetric_and_diagonal():
+    k, n, s2 = 6, 6, 0
+    h, eri = random_dense(k, 3)
+    ham = dmrg.Ham(h, eri)
+    i = 2
+    mps = random_mps(k, n, s2, 6, seed=1, gauge="LR:%d" % i)
+    H = dmrg.Heff(dmrg.build_left(mps, ham, i)[-1], dmrg.build_right(mps, ham, i + 2)[i + 2], ham, i)
+    M = np.stack([H.apply(e) for e in np.eye(H.nnz)], axis=1)
+    assert np.abs(M - M.T).max() < 1e-12
+    assert np.abs(np.diag(M) - H.diagonal()).max() < 1e-12
+
+
+def test_davidson_against_dense_eigh():
+    rng = np.random.default_rng(5)
+    n = 200
+    M = rng.normal(size=(n, n))
+    M = M + M.T + np.diag(np.arange(n) * 2.0)
+    w = np.linalg.eigvalsh(M)
+    th, u, nmv, rn, ok = dmrg.davidson(lambda v: M @ v, np.diag(M).copy(), rng.normal(size=n), tol=1e-10,
+                                       max_iter=300)
+    assert ok and abs(th - w[0]) < 1e-10 and np.linalg.norm(M @ u - th * u) < 1e-9
+
+
+def test_truncation_never_splits_a_degenerate_cluster():
+    # one left sector (dim 1 bond 0), theta = diag-like with singular values 0.8, 0.5, 0.5(degenerate), 0.1:
+    # D = 2 would cut through the 0.5 doublet -> rule keeps 1 (reading S14)
+    bonds_l = [(0, 0, 4)]
+    bonds_r = [(0, 0, 4)]
+    sv = np.array([0.8, 0.5, 0.5 * (1 - 1e-9), 0.1])
+    sv = sv / np.linalg.norm(sv)
+    rng = np.random.default_rng(0)
+    U, _ = np.linalg.qr(rng.normal(size=(4, 4)))
+    V, _ = np.linalg.qr(rng.normal(size=(4, 4)))
+    theta = {(0, 0, 0): U @ np.diag(sv) @ V.T}
+    mid, A, B, trunc, kept = dmrg.split_theta(theta, bonds_l, bonds_r, 2, "fwd")
+    assert kept == 1 and mid == [(0, 0, 1)]
+    assert abs(trunc - (1 - sv[0] ** 2)) < 1e-12
+    mid, A, B, trunc, kept = dmrg.split_theta(theta, bonds_l, bonds_r, 3, "fwd")
+    assert kept == 3 and abs(trunc - sv[3] ** 2) < 1e-12
+    assert np.abs(A[(0, 0)].T @ A[(0, 0)] - np.eye(3)).max() < 1e-12       # left-orthonormal
+    assert abs(np.sum(B[(0, 0)] ** 2) - 1.0) < 1e-12                        # kept state renormalised
+
+
+@pytest.mark.parametrize("k,n,s2", [(5, 5, 1), (6, 6, 0)])
+def test_untruncated_sweep_reaches_fci_energy_and_rdms(k, n, s2):
+    h, eri = random_dense(k, 11 + k, scale=0.25)
+    sp = fci.FCISpace(k, n, s2)
+    e0, c0 = sp.ground_state(h, eri)
+    mps = random_mps(k, n, s2, 8, seed=2, gauge="R")
+    eng = dmrg.SweepEngine(h, eri, mps, davidson_tol=1e-11, davidson_max_iter=300)
+    for _ in range(3):
+        r = eng.sweep(10 ** 6)
+    assert abs(r["energy_last"] - e0) < 1e-10
+    g, G = dmrg.rdm12(h, eri, eng.mps)
+    gf, Gf = sp.rdm12(c0)
+    assert np.abs(g - gf).max() < 1e-8 and np.abs(G - Gf).max() < 1e-8     # eigenvector accuracy ~ sqrt-free 1e-10/gap
+    assert abs(np.einsum("pq,pq", h, g) + 0.5 * np.einsum("pqrs,pqrs", eri, G) - e0) < 1e-10
+
+
+def test_truncated_sweep_variational_and_rdm_energy_of_final_mps():
+    k, n, s2, D = 6, 6, 0, 10
+    h, eri = random_dense(k, 17, scale=0.25)
+    sp = fci.FCISpace(k, n, s2)
+    e0, _ = sp.ground_state(h, eri)
+    mps = random_mps(k, n, s2, D, seed=2, gauge="R")
+    eng = dmrg.SweepEngine(h, eri, mps, davidson_tol=1e-10, davidson_max_iter=300)
+    for _ in range(2):
+        r = eng.sweep(D)
+    assert all(b["energy"] >= e0 - 1e-10 for b in r["bonds"])
+    assert max(sum(d for _, _, d in bb) for bb in eng.mps["bonds"]) <= D
+    c = fci.mps_to_ci(eng.mps, sp)
+    assert abs(np.linalg.norm(c) - 1.0) < 1e-10
+    e_mps = c @ sp.apply_h(h, eri, c)
+    g, G = dmrg.rdm12(h, eri, eng.mps)
+    assert abs(np.einsum("pq,pq", h, g) + 0.5 * np.einsum("pqrs,pqrs", eri, G) - e_mps) < 1e-10     # reading S20
+    gf, Gf = sp.rdm12(c)
+    assert np.abs(g - gf).max() < 1e-11 and np.abs(G - Gf).max() < 1e-11
+
+
+def test_rdm_invariants_random_mps():
+    k, n, s2 = 7, 9, 1
+    h, eri = random_dense(k, 1)
+    mps = random_mps(k, n, s2, 14, seed=8, gauge="R")
+    g, G = dmrg.rdm12(h, eri, mps)
+    assert abs(np.trace(g) - n) < 1e-11
+    assert np.abs(np.einsum("pqrr->pq", G) - (n - 1) * g).max() < 1e-11
+    assert np.abs(G - G.transpose(2, 3, 0, 1)).max() < 1e-11
+    assert np.abs(G - G.transpose(1, 0, 3, 2)).max() < 1e-11
+    assert np.abs(g - g.T).max() < 1e-12
+
+
+@pytest.mark.slow
+def test_config1_untruncated_sweep_vs_fci():
+    cfg = make_config(1)
+    k = cfg["k"]
+    mps = random_mps(k, cfg["n_elec"], 0, 64, seed=cfg["seed"] + 1000, gauge="R")
+    eng = dmrg.SweepEngine(cfg["h"], cfg["eri"], mps, davidson_tol=1e-10)
+    for _ in range(3):
+        r = eng.sweep(1024)
+    assert abs(r["energy_last"] + cfg["e_core"] - (-0.8822829988)) < 1e-8
