@@ -1,0 +1,317 @@
+// C ABI of include/dmrg_b200.h: argument checking, host<->device marshalling, exception -> status translation.
+#include <cmath>
+#include <cstring>
+
+#include "../../include/dmrg_b200.h"
+#include "core.hpp"
+
+using namespace dmrg;
+
+struct dmrg_ctx {
+    Engine eng;
+};
+
+namespace dmrg {
+
+void Engine::ensure_left(int i) {
+    if (L.find(0) == L.end()) L[0] = empty_block('L', k, mps);
+    for (int b = 0; b < i; ++b) {
+        if (L.find(b + 1) != L.end()) continue;
+        L[b + 1] = grow(*L[b], ham, mps, mode_L(b + 1), *this);
+        if (!keep_env_stack && b > 0) L.erase(b);
+    }
+}
+void Engine::ensure_right(int j) {
+    if (R.find(k) == R.end()) R[k] = empty_block('R', k, mps);
+    for (int b = k; b > j; --b) {
+        if (R.find(b - 1) != R.end()) continue;
+        R[b - 1] = grow(*R[b], ham, mps, mode_R(b - 1), *this);
+        if (!keep_env_stack && b < k) R.erase(b);
+    }
+}
+void Engine::prepare_bond(int i) {
+    plan.reset();
+    ensure_left(i);
+    ensure_right(i + 2);
+    plan = build_heff(ham, *L[i], *R[i + 2], i, *this);
+}
+HeffPlan::~HeffPlan() {
+    if (X) X->drop_temps();
+}
+
+}  // namespace dmrg
+
+#define API_BEGIN(ctx)                                   \
+    if (!(ctx)) return DMRG_EINVAL;                      \
+    Engine& eng = (ctx)->eng;                            \
+    try {
+#define API_END                                          \
+    }                                                    \
+    catch (const Error& e) { eng.last_error = e.what(); return e.code; }                 \
+    catch (const std::bad_alloc&) { eng.last_error = "host memory exhausted"; return DMRG_ENOMEM; } \
+    catch (const std::exception& e) { eng.last_error = e.what(); return DMRG_ESTATE; }
+
+static int fail(Engine& eng, int code, const char* msg) {
+    eng.last_error = msg;
+    return code;
+}
+
+extern "C" {
+
+void dmrg_default_options(dmrg_options* o) {
+    if (!o) return;
+    Options d;
+    o->davidson_tol = d.davidson_tol;
+    o->davidson_max_iter = d.davidson_max_iter;
+    o->davidson_max_subspace = d.davidson_max_subspace;
+    o->sv_floor = d.sv_floor;
+    o->cluster_rel_gap = d.cluster_rel_gap;
+    o->device_id = 0;
+    o->keep_env_stack = 1;
+    o->workspace_bytes = 0;
+}
+
+int dmrg_create(dmrg_ctx** out, int k, int n_elec, int two_sz, const double* h, const double* eri,
+                const dmrg_options* opt) {
+    if (!out || !h || !eri) return DMRG_EINVAL;
+    *out = nullptr;
+    if (k < 1 || k > 120 || n_elec < 0 || n_elec > 2 * k) return DMRG_EINVAL;
+    if (((n_elec + two_sz) & 1) != 0) return DMRG_EINVAL;
+    const int na = (n_elec + two_sz) / 2, nb = (n_elec - two_sz) / 2;
+    if (na < 0 || nb < 0 || na > k || nb > k) return DMRG_EINVAL;
+    for (int p = 0; p < k; ++p)
+        for (int q = 0; q < p; ++q)
+            if (std::fabs(h[p * k + q] - h[q * k + p]) > 1e-12) return DMRG_EINVAL;
+    dmrg_ctx* ctx = nullptr;
+    try {
+        ctx = new dmrg_ctx();
+        Engine& eng = ctx->eng;
+        if (opt) {
+            eng.opt.davidson_tol = opt->davidson_tol;
+            eng.opt.davidson_max_iter = opt->davidson_max_iter;
+            eng.opt.davidson_max_subspace = opt->davidson_max_subspace;
+            eng.opt.sv_floor = opt->sv_floor;
+            eng.opt.cluster_rel_gap = opt->cluster_rel_gap;
+            eng.opt.device_id = opt->device_id;
+            eng.opt.workspace_bytes = opt->workspace_bytes;
+            eng.keep_env_stack = opt->keep_env_stack != 0;
+        }
+        if (eng.opt.davidson_max_subspace < 2 || eng.opt.davidson_max_subspace > COMBINE_MAX ||
+            eng.opt.davidson_max_iter < 1 || !(eng.opt.davidson_tol > 0)) { delete ctx; return DMRG_EINVAL; }
+        int ndev = 0;
+        if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= eng.opt.device_id) { delete ctx; return DMRG_ECUDA; }
+        cuda_check(cudaSetDevice(eng.opt.device_id), "cudaSetDevice");
+        cuda_check(cudaStreamCreateWithFlags(&eng.stream, cudaStreamNonBlocking), "cudaStreamCreate");
+        eng.k = k; eng.n_elec = n_elec; eng.two_sz = two_sz;
+        eng.bsw = (k >= 3) ? (k - 3) / 2 : -1;
+        eng.ham.k = k;
+        eng.ham.h.assign(h, h + (size_t)k * k);
+        eng.ham.eri.assign(eri, eri + (size_t)k * k * k * k);
+        eng.svd = svd_create(eng.stream);
+    } catch (...) {
+        delete ctx;
+        return DMRG_ECUDA;
+    }
+    *out = ctx;
+    return DMRG_OK;
+}
+
+int dmrg_destroy(dmrg_ctx* ctx) {
+    if (!ctx) return DMRG_EINVAL;
+    Engine& eng = ctx->eng;
+    eng.plan.reset();
+    eng.L.clear();
+    eng.R.clear();
+    eng.mps.sites.clear();
+    if (eng.svd) svd_destroy(eng.svd);
+    if (eng.stream) cudaStreamDestroy(eng.stream);
+    delete ctx;
+    return DMRG_OK;
+}
+
+const char* dmrg_last_error(const dmrg_ctx* ctx) { return ctx ? ctx->eng.last_error.c_str() : "null context"; }
+int64_t dmrg_launch_count(const dmrg_ctx* ctx) { return ctx ? ctx->eng.launches : 0; }
+int64_t dmrg_device_bytes(const dmrg_ctx*) { return g_device_bytes; }
+
+int dmrg_mps_import(dmrg_ctx* ctx, const dmrg_mps_blob* b) {
+    API_BEGIN(ctx)
+    if (!b || !b->bond_ptr || !b->sec_n || !b->sec_2sz || !b->sec_dim || !b->blk_ptr || !b->blk_l || !b->blk_s ||
+        !b->blk_off || !b->data || !b->gauge)
+        return fail(eng, DMRG_EINVAL, "mps_import: null array");
+    const int k = eng.k;
+    if (b->k != k || b->n_elec != eng.n_elec || b->two_sz != eng.two_sz)
+        return fail(eng, DMRG_EINVAL, "mps_import: k / n_elec / two_sz differ from the context");
+    MPS m;
+    m.k = k; m.n_elec = eng.n_elec; m.two_sz = eng.two_sz;
+    m.bonds.resize(k + 1);
+    for (int bd = 0; bd <= k; ++bd) {
+        for (int j = b->bond_ptr[bd]; j < b->bond_ptr[bd + 1]; ++j) {
+            Sector s{b->sec_n[j], b->sec_2sz[j], b->sec_dim[j]};
+            if (s.d < 1) return fail(eng, DMRG_EINVAL, "mps_import: sector of dimension < 1");
+            if (!m.bonds[bd].empty()) {
+                const Sector& pr = m.bonds[bd].back();
+                if (!(pr.n < s.n || (pr.n == s.n && pr.s < s.s))) return fail(eng, DMRG_EINVAL, "mps_import: sectors not sorted");
+            }
+            m.bonds[bd].push_back(s);
+        }
+        if (m.bonds[bd].empty()) return fail(eng, DMRG_EINVAL, "mps_import: empty bond");
+    }
+    if (m.bonds[0].size() != 1 || m.bonds[0][0].n != 0 || m.bonds[0][0].s != 0 || m.bonds[0][0].d != 1 ||
+        m.bonds[k].size() != 1 || m.bonds[k][0].n != eng.n_elec || m.bonds[k][0].s != eng.two_sz || m.bonds[k][0].d != 1)
+        return fail(eng, DMRG_EINVAL, "mps_import: boundary bonds must be {(0,0,1)} and {(n_elec,two_sz,1)}");
+    m.sites.resize(k);
+    for (int p = 0; p < k; ++p) {
+        SiteTensor& t = m.sites[p];
+        make_site_tensor(t, m.bonds[p], m.bonds[p + 1]);
+        t.gauge = (char)b->gauge[p];
+        if (t.gauge != 'L' && t.gauge != 'R' && t.gauge != 'C') return fail(eng, DMRG_EINVAL, "mps_import: bad gauge flag");
+        if (t.nnz) cuda_check(cudaMemsetAsync(t.data.p, 0, (size_t)t.nnz * 8, eng.stream), "memset");
+        std::vector<char> seen(t.blocks.size(), 0);
+        for (int j = b->blk_ptr[p]; j < b->blk_ptr[p + 1]; ++j) {
+            const int l = b->blk_l[j], s = b->blk_s[j];
+            if (l < 0 || l >= (int)m.bonds[p].size() || s < 0 || s > 3) return fail(eng, DMRG_EINVAL, "mps_import: bad block index");
+            const int idx = t.lookup[l * 4 + s];
+            if (idx < 0) return fail(eng, DMRG_EINVAL, "mps_import: block whose right sector does not exist");
+            const SiteTensor::Blk& bk = t.blocks[idx];
+            seen[idx] = 1;
+            cuda_check(cudaMemcpy2DAsync(bk.ptr, (size_t)bk.ld * 8, b->data + b->blk_off[j], (size_t)bk.cols * 8,
+                                         (size_t)bk.cols * 8, bk.rows, cudaMemcpyHostToDevice, eng.stream), "mps upload");
+        }
+    }
+    cuda_check(cudaStreamSynchronize(eng.stream), "mps upload");
+    eng.invalidate();
+    eng.mps = std::move(m);
+    eng.have_mps = true;
+    return DMRG_OK;
+    API_END
+}
+
+int dmrg_mps_export(dmrg_ctx* ctx, dmrg_mps_blob* b) {
+    API_BEGIN(ctx)
+    if (!b) return fail(eng, DMRG_EINVAL, "mps_export: null blob");
+    if (!eng.have_mps) return fail(eng, DMRG_ESTATE, "mps_export: no MPS");
+    const MPS& m = eng.mps;
+    int64_t ns = 0, nb = 0, nd = 0;
+    for (auto& bd : m.bonds) ns += (int64_t)bd.size();
+    for (auto& t : m.sites)
+        for (auto& bk : t.blocks) { nb++; nd += (int64_t)bk.rows * bk.cols; }
+    b->k = m.k; b->n_elec = m.n_elec; b->two_sz = m.two_sz;
+    if (!b->data) { b->n_sectors = ns; b->n_blocks = nb; b->n_data = nd; return DMRG_OK; }
+    if (b->n_sectors < ns || b->n_blocks < nb || b->n_data < nd) return fail(eng, DMRG_EINVAL, "mps_export: arrays too small");
+    int32_t* bond_ptr = (int32_t*)b->bond_ptr; int32_t* sn = (int32_t*)b->sec_n; int32_t* ss = (int32_t*)b->sec_2sz;
+    int32_t* sd = (int32_t*)b->sec_dim; int32_t* blk_ptr = (int32_t*)b->blk_ptr; int32_t* bl = (int32_t*)b->blk_l;
+    int32_t* bs = (int32_t*)b->blk_s; int64_t* bo = (int64_t*)b->blk_off; double* data = (double*)b->data;
+    uint8_t* gauge = (uint8_t*)b->gauge;
+    int j = 0;
+    bond_ptr[0] = 0;
+    for (int bd = 0; bd <= m.k; ++bd) {
+        for (const Sector& s : m.bonds[bd]) { sn[j] = s.n; ss[j] = s.s; sd[j] = s.d; ++j; }
+        bond_ptr[bd + 1] = j;
+    }
+    j = 0;
+    int64_t off = 0;
+    blk_ptr[0] = 0;
+    for (int p = 0; p < m.k; ++p) {
+        for (const auto& bk : m.sites[p].blocks) {
+            bl[j] = bk.l; bs[j] = bk.s; bo[j] = off;
+            cuda_check(cudaMemcpy2DAsync(data + off, (size_t)bk.cols * 8, bk.ptr, (size_t)bk.ld * 8, (size_t)bk.cols * 8,
+                                         bk.rows, cudaMemcpyDeviceToHost, eng.stream), "mps download");
+            off += (int64_t)bk.rows * bk.cols;
+            ++j;
+        }
+        blk_ptr[p + 1] = j;
+        gauge[p] = (uint8_t)m.sites[p].gauge;
+    }
+    cuda_check(cudaStreamSynchronize(eng.stream), "mps download");
+    b->n_sectors = ns; b->n_blocks = nb; b->n_data = nd;
+    return DMRG_OK;
+    API_END
+}
+
+int dmrg_prepare_bond(dmrg_ctx* ctx, int i) {
+    API_BEGIN(ctx)
+    if (!eng.have_mps) return fail(eng, DMRG_ESTATE, "prepare_bond: import an MPS first");
+    if (i < 0 || i > eng.k - 2) return fail(eng, DMRG_EINVAL, "prepare_bond: bond out of range");
+    eng.sweep_ready = false;
+    eng.prepare_bond(i);
+    return DMRG_OK;
+    API_END
+}
+
+static int need_plan(Engine& eng, int i) {
+    if (!eng.plan || eng.plan->bond != i) return fail(eng, DMRG_ESTATE, "bond not prepared (call dmrg_prepare_bond)");
+    return DMRG_OK;
+}
+
+int dmrg_heff_layout(dmrg_ctx* ctx, int i, int64_t* nnz, int32_t* nblocks, dmrg_block* blocks) {
+    API_BEGIN(ctx)
+    if (int rc = need_plan(eng, i)) return rc;
+    const HeffPlan& p = *eng.plan;
+    if (nnz) *nnz = p.nnz;
+    if (nblocks) *nblocks = (int32_t)p.layout.size();
+    if (blocks)
+        for (size_t j = 0; j < p.layout.size(); ++j) {
+            const PsiBlock& b = p.layout[j];
+            blocks[j].l_idx = b.l; blocks[j].s_i = b.ab >> 2; blocks[j].s_j = b.ab & 3; blocks[j].r_idx = b.r;
+            blocks[j].rows = b.rows; blocks[j].cols = b.cols; blocks[j].offset = b.off;
+        }
+    return DMRG_OK;
+    API_END
+}
+
+int dmrg_heff_apply(dmrg_ctx* ctx, int i, const double* x, double* y, int where, void* cuda_stream) {
+    API_BEGIN(ctx)
+    if (int rc = need_plan(eng, i)) return rc;
+    if (!x || !y) return fail(eng, DMRG_EINVAL, "heff_apply: null vector");
+    HeffPlan& p = *eng.plan;
+    const size_t bytes = (size_t)p.nnz * 8;
+    if (where == DMRG_HOST) {
+        cuda_check(cudaMemcpyAsync(p.xbuf.p, x, bytes, cudaMemcpyHostToDevice, eng.stream), "x upload");
+        heff_apply(p, p.xbuf.p, p.ybuf.p, eng);
+        cuda_check(cudaMemcpyAsync(y, p.ybuf.p, bytes, cudaMemcpyDeviceToHost, eng.stream), "y download");
+        cuda_check(cudaStreamSynchronize(eng.stream), "heff_apply");
+    } else if (where == DMRG_DEVICE) {
+        // order the library stream after the caller's stream and back (events), so device buffers are used in place
+        cudaStream_t cs = (cudaStream_t)cuda_stream;
+        cudaEvent_t ev;
+        cuda_check(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming), "event");
+        cuda_check(cudaEventRecord(ev, cs), "event record");
+        cuda_check(cudaStreamWaitEvent(eng.stream, ev, 0), "stream wait");
+        heff_apply(p, x, y, eng);
+        cuda_check(cudaEventRecord(ev, eng.stream), "event record");
+        cuda_check(cudaStreamWaitEvent(cs, ev, 0), "stream wait");
+        cuda_check(cudaEventDestroy(ev), "event destroy");
+    } else return fail(eng, DMRG_EINVAL, "heff_apply: bad `where`");
+    return DMRG_OK;
+    API_END
+}
+
+int dmrg_heff_diag(dmrg_ctx* ctx, int i, double* d, int where, void* cuda_stream) {
+    API_BEGIN(ctx)
+    (void)cuda_stream;
+    if (int rc = need_plan(eng, i)) return rc;
+    if (!d) return fail(eng, DMRG_EINVAL, "heff_diag: null vector");
+    HeffPlan& p = *eng.plan;
+    if (where == DMRG_HOST) {
+        heff_diag(p, p.ybuf.p, eng);
+        cuda_check(cudaMemcpyAsync(d, p.ybuf.p, (size_t)p.nnz * 8, cudaMemcpyDeviceToHost, eng.stream), "diag download");
+    } else heff_diag(p, d, eng);
+    cuda_check(cudaStreamSynchronize(eng.stream), "heff_diag");
+    return DMRG_OK;
+    API_END
+}
+
+int dmrg_heff_stats(dmrg_ctx* ctx, int i, double* f_alg, double* f_exec, double* b_alg, int64_t* nterms, int64_t* ngemm) {
+    API_BEGIN(ctx)
+    if (int rc = need_plan(eng, i)) return rc;
+    const HeffPlan& p = *eng.plan;
+    if (f_alg) *f_alg = p.f_alg;
+    if (f_exec) *f_exec = p.f_exec;
+    if (b_alg) *b_alg = p.b_alg;
+    if (nterms) *nterms = p.nterms;
+    if (ngemm) *ngemm = p.ngemm;
+    return DMRG_OK;
+    API_END
+}
+
+}  // extern "C"

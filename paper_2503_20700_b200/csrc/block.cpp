@@ -1,0 +1,290 @@
+// Device-resident block operators: storage, launch-descriptor plumbing, linear combinations, blocking (grow).
+#include <algorithm>
+#include <cassert>
+#include <cstdio>
+
+#include "core.hpp"
+
+namespace dmrg {
+
+// ---------------------------------------------------------------------------------------------------------------
+// device memory and descriptors
+// ---------------------------------------------------------------------------------------------------------------
+int64_t g_device_bytes = 0;
+static std::unordered_map<void*, size_t> g_sizes;
+
+void cuda_check(cudaError_t e, const char* what) {
+    if (e != cudaSuccess) throw Error(-4, std::string(what) + ": " + cudaGetErrorString(e));
+}
+void* dev_alloc(size_t bytes) {
+    void* p = nullptr;
+    if (bytes == 0) return nullptr;
+    cudaError_t e = cudaMalloc(&p, bytes);
+    if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); throw Error(-3, "out of device memory"); }
+    cuda_check(e, "cudaMalloc");
+    g_sizes[p] = bytes;
+    g_device_bytes += (int64_t)bytes;
+    return p;
+}
+void dev_free(void* p) {
+    if (!p) return;
+    auto it = g_sizes.find(p);
+    if (it != g_sizes.end()) { g_device_bytes -= (int64_t)it->second; g_sizes.erase(it); }
+    cudaFree(p);
+}
+
+int find_sector(const Basis& b, int n, int s) {
+    int lo = 0, hi = (int)b.size() - 1;
+    while (lo <= hi) {
+        const int mid = (lo + hi) / 2;
+        if (b[mid].n == n && b[mid].s == s) return mid;
+        if (b[mid].n < n || (b[mid].n == n && b[mid].s < s)) lo = mid + 1;
+        else hi = mid - 1;
+    }
+    return -1;
+}
+
+void make_site_tensor(SiteTensor& t, const Basis& bl, const Basis& br) {
+    t.blocks.clear();
+    t.lookup.assign(bl.size() * 4, -1);
+    int64_t off = 0;
+    std::vector<int64_t> offs;
+    for (int l = 0; l < (int)bl.size(); ++l)
+        for (int s = 0; s < 4; ++s) {
+            const int r = find_sector(br, bl[l].n + SITE_QN[s], bl[l].s + SITE_QS[s]);
+            if (r < 0) continue;
+            t.lookup[l * 4 + s] = (int)t.blocks.size();
+            t.blocks.push_back({l, s, r, bl[l].d, br[r].d, pad2(br[r].d), nullptr});
+            offs.push_back(off);
+            off += (int64_t)bl[l].d * pad2(br[r].d);          // even leading dimension: 16-byte aligned rows
+        }
+    t.data.alloc((size_t)off);
+    t.nnz = off;
+    for (size_t j = 0; j < t.blocks.size(); ++j) t.blocks[j].ptr = t.data.p + offs[j];
+}
+
+int GemmBatch::add_task(double* C, int ldc, int M, int N, int flags) {
+    Task t;
+    t.C = C; t.ldc = ldc; t.M = M; t.N = N; t.seg_begin = 0; t.seg_count = 0; t.flags = flags;
+    tasks.push_back(t);
+    return (int)tasks.size() - 1;
+}
+void GemmBatch::add_seg(int task, const double* A, int lda, const double* B, int ldb, int K, int flags,
+                        double alpha) {
+    Seg s;
+    s.A = A; s.B = B; s.lda = lda; s.ldb = ldb; s.K = K; s.flags = flags; s.alpha = alpha;
+    segs.push_back(s);
+    seg_task.push_back(task);
+    if (!(flags & SEG_IDENT_B)) flops += 2.0 * tasks[task].M * (double)tasks[task].N * K;
+}
+
+void finalize(GemmBatch& b, GemmLaunch& out, Engine& eng) {
+    const int nt = (int)b.tasks.size();
+    for (auto& t : b.tasks) t.seg_count = 0;
+    for (int t : b.seg_task) b.tasks[t].seg_count++;
+    int run = 0;
+    for (auto& t : b.tasks) { t.seg_begin = run; run += t.seg_count; }
+    std::vector<Seg> sorted(b.segs.size());
+    std::vector<int> cursor(nt);
+    for (int t = 0; t < nt; ++t) cursor[t] = b.tasks[t].seg_begin;
+    for (size_t j = 0; j < b.segs.size(); ++j) sorted[cursor[b.seg_task[j]]++] = b.segs[j];   // stable
+    // tiles, heaviest tasks first so that the tail of the launch is made of short tiles
+    std::vector<double> weight(nt, 0.0);
+    for (int t = 0; t < nt; ++t)
+        for (int j = 0; j < b.tasks[t].seg_count; ++j) weight[t] += sorted[b.tasks[t].seg_begin + j].K;
+    std::vector<int> order(nt);
+    for (int t = 0; t < nt; ++t) order[t] = t;
+    std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return weight[x] > weight[y]; });
+    std::vector<Tile> tiles;
+    for (int t : order) {
+        const Task& tk = b.tasks[t];
+        if (tk.M <= 0 || tk.N <= 0) continue;
+        const int nm = (tk.M + GEMM_BM - 1) / GEMM_BM, nn = (tk.N + GEMM_BN - 1) / GEMM_BN;
+        for (int i = 0; i < nm; ++i)
+            for (int j = 0; j < nn; ++j) tiles.push_back({t, i, j});
+    }
+    out.tasks.upload(b.tasks, eng.stream);
+    out.segs.upload(sorted, eng.stream);
+    out.tiles.upload(tiles, eng.stream);
+    out.ntiles = (int)tiles.size();
+    out.flops = b.flops;
+    cuda_check(cudaStreamSynchronize(eng.stream), "descriptor upload");   // host vectors die after this call
+}
+void run(const GemmLaunch& l, Engine& eng) {
+    if (l.ntiles == 0) return;
+    launch_seg_gemm(l.tasks.p, l.segs.p, l.tiles.p, l.ntiles, eng.stream);
+    eng.launches++;
+}
+void run_once(GemmBatch& b, Engine& eng) {
+    if (b.tasks.empty()) return;
+    GemmLaunch l;
+    finalize(b, l, eng);
+    run(l, eng);
+    cuda_check(cudaStreamSynchronize(eng.stream), "grouped GEMM");
+    b = GemmBatch();
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Block
+// ---------------------------------------------------------------------------------------------------------------
+Block::Block(char side_, int b_, int k_, const Basis& basis_, char mode_)
+    : side(side_), b(b_), k(k_), mode(mode_), basis(basis_) {}
+Block::~Block() {
+    for (void* p : allocs) dev_free(p);
+    for (void* p : temp_allocs) dev_free(p);
+}
+std::vector<int> Block::inside() const {
+    std::vector<int> v;
+    if (side == 'L') for (int P = 0; P < 2 * b; ++P) v.push_back(P);
+    else for (int P = 2 * b; P < 2 * k; ++P) v.push_back(P);
+    return v;
+}
+std::vector<int> Block::outside() const {
+    std::vector<int> v;
+    if (side == 'L') for (int P = 2 * b; P < 2 * k; ++P) v.push_back(P);
+    else for (int P = 0; P < 2 * b; ++P) v.push_back(P);
+    return v;
+}
+const OpRef& Block::get(const Label& l) const {
+    auto it = ops.find(l.key());
+    if (it == ops.end()) {
+        char buf[96];
+        std::snprintf(buf, sizeof buf, "operator (%d,%d,%d,%d) missing on block %c%d", l.kind, l.a, l.b, l.c, side, b);
+        throw std::logic_error(buf);
+    }
+    return it->second;
+}
+int Block::class_of(int dn, int ds) {
+    for (size_t c = 0; c < classes.size(); ++c)
+        if (classes[c].dn == dn && classes[c].ds == ds) return (int)c;
+    OpClass oc;
+    oc.dn = dn; oc.ds = ds;
+    const int ns = (int)basis.size();
+    oc.out.assign(ns, -1); oc.inv.assign(ns, -1); oc.off.assign(ns, 0);
+    int64_t off = 0;
+    for (int i = 0; i < ns; ++i) {
+        const int o = find_sector(basis, basis[i].n + dn, basis[i].s + ds);
+        if (o < 0) continue;
+        oc.out[i] = o; oc.inv[o] = i; oc.off[i] = off;
+        off += (int64_t)basis[o].d * pad2(basis[i].d);         // even leading dimension: 16-byte aligned rows
+    }
+    oc.nnz = off; oc.ld = off;
+    classes.push_back(oc);
+    return (int)classes.size() - 1;
+}
+int Block::label_class(const Label& l) {
+    int dn, ds;
+    op_shift(l, dn, ds);
+    return class_of(g() * dn, g() * ds);
+}
+void Block::allocate(const std::vector<Label>& labels, bool temp) {
+    std::map<std::pair<int, int>, int> group;                  // (kind, class) -> new stack index
+    const size_t first = stacks.size();
+    for (const Label& l : labels) {
+        if (has(l)) throw std::logic_error("Block::allocate: operator exists");
+        const int cls = label_class(l);
+        auto key = std::make_pair(l.kind, cls);
+        auto it = group.find(key);
+        if (it == group.end()) {
+            Stack s; s.kind = l.kind; s.cls = cls;
+            stacks.push_back(s);
+            it = group.emplace(key, (int)stacks.size() - 1).first;
+        }
+        Stack& st = stacks[it->second];
+        OpRef r; r.cls = cls; r.stack = it->second; r.row = (int)st.members.size();
+        st.members.push_back(l);
+        ops[l.key()] = r;
+        if (temp) temp_keys.push_back(l.key());
+    }
+    int64_t total = 0;
+    for (size_t s = first; s < stacks.size(); ++s) total += (int64_t)stacks[s].members.size() * classes[stacks[s].cls].ld;
+    double* base = (double*)dev_alloc((size_t)total * sizeof(double));
+    if (base) {
+        (temp ? temp_allocs : allocs).push_back(base);
+        cuda_check(cudaMemset(base, 0, (size_t)total * sizeof(double)), "memset");   // padding stays finite
+    }
+    bytes_ += total * 8;
+    int64_t off = 0;
+    for (size_t s = first; s < stacks.size(); ++s) {
+        Stack& st = stacks[s];
+        st.base = base ? base + off : nullptr;
+        const int64_t ld = classes[st.cls].ld;
+        for (size_t r = 0; r < st.members.size(); ++r) ops[st.members[r].key()].ptr = st.base ? st.base + (int64_t)r * ld : nullptr;
+        off += (int64_t)st.members.size() * ld;
+    }
+}
+void Block::drop_temps() {
+    for (uint32_t key : temp_keys) ops.erase(key);
+    temp_keys.clear();
+    for (void* p : temp_allocs) dev_free(p);
+    temp_allocs.clear();
+}
+int64_t Block::bytes() const { return bytes_; }
+
+bool op_block(const Block& blk, const OpRef& op, bool trans, int in, OpBlockView& v) {
+    const OpClass& c = blk.classes[op.cls];
+    if (!trans) {
+        const int o = c.out[in];
+        if (o < 0) return false;
+        v.out = o; v.ptr = op.ptr + c.off[in]; v.ld = pad2(blk.basis[in].d); v.trans = false;
+        v.rows = blk.basis[o].d; v.cols = blk.basis[in].d;
+    } else {
+        const int j = c.inv[in];                               // stored block j -> in ; transposed maps in -> j
+        if (j < 0) return false;
+        v.out = j; v.ptr = op.ptr + c.off[j]; v.ld = pad2(blk.basis[j].d); v.trans = true;
+        v.rows = blk.basis[j].d; v.cols = blk.basis[in].d;
+    }
+    return true;
+}
+
+static bool block_has_op(const void* blk, const Label& l) { return ((const Block*)blk)->has(l); }
+BlockInfo block_info(const Block& b) {
+    BlockInfo bi;
+    bi.side = b.side; bi.inside = b.inside(); bi.has_op = block_has_op; bi.blk = &b;
+    return bi;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// linear combinations of operator stacks as GEMMs:  Dst[n_dst x nnz] (+)= W[n_dst x n_src] Src[n_src x nnz]
+// ---------------------------------------------------------------------------------------------------------------
+void lincomb(Block& blk, const std::vector<LinSpec>& specs, bool accumulate, Engine& eng) {
+    std::map<int, std::vector<const LinSpec*>> by_stack;       // dst stack -> specs
+    for (const LinSpec& s : specs) by_stack[blk.get(s.dst).stack].push_back(&s);
+    GemmBatch batch;
+    std::vector<DevVec<double>> keep;
+    for (auto& kv : by_stack) {
+        const Stack& ds = blk.stacks[kv.first];
+        const OpClass& cls = blk.classes[ds.cls];
+        int src_stack = -1;
+        for (const LinSpec* s : kv.second)
+            for (const LinItem& it : s->items) {
+                const int st = blk.get(it.src).stack;
+                if (src_stack >= 0 && st != src_stack) throw std::logic_error("lincomb: sources span two stacks");
+                src_stack = st;
+            }
+        const int n_dst = (int)ds.members.size();
+        if (!accumulate && (int)kv.second.size() != n_dst) throw std::logic_error("lincomb: partial overwrite");
+        if (cls.nnz == 0) continue;
+        if (src_stack < 0) {                                   // nothing to add
+            if (!accumulate) cuda_check(cudaMemsetAsync(ds.base, 0, (size_t)n_dst * cls.ld * 8, eng.stream), "memset");
+            continue;
+        }
+        const Stack& ss = blk.stacks[src_stack];
+        if (ss.cls != ds.cls) throw std::logic_error("lincomb: class mismatch");
+        const int n_src = (int)ss.members.size();
+        std::vector<double> W((size_t)n_dst * n_src, 0.0);
+        for (const LinSpec* s : kv.second) {
+            const int r = blk.get(s->dst).row;
+            for (const LinItem& it : s->items) W[(size_t)r * n_src + blk.get(it.src).row] += it.coef;
+        }
+        keep.emplace_back();
+        keep.back().upload(W, eng.stream);
+        cuda_check(cudaStreamSynchronize(eng.stream), "lincomb upload");
+        // the row length can exceed the int range of Task::N only beyond 2^31 doubles per operator: not reachable
+        const int t = batch.add_task(ds.base, (int)cls.ld, n_dst, (int)cls.nnz, accumulate ? TASK_ACCUM : 0);
+        batch.add_seg(t, keep.back().p, n_src, ss.base, (int)cls.ld, n_src, 0, 1.0);
+    }
+    run_once(batch, eng);
+}
+
+}  // namespace dmrg

@@ -1,0 +1,314 @@
+// Operator renormalisation (blocking), SURVEY.md 8(a) row a5 / DESIGN.md "Algorithm" step 3:
+//   X' = sum_{s',s} A[s']^T ( sum_j c_j O_j (x) o_j[s',s] ) A[s]      (left block; B ... B^T for a right block)
+// The enlarged operator is never materialised: phase 1 forms the half-rotated pieces
+//   tmp[(o,s'), m] = sum_{j,s,i} c_j o_j[s',s] sgn  O_j[o<-i] A[(i,s) -> m]      (K-concatenated over pieces)
+// and phase 2 contracts them with the bra tensor, out[m' <- m] = sum_{(o,s')} A[(o,s') -> m']^T tmp[(o,s'), m];
+// both phases are launches of the grouped FP64 GEMM kernel over all new operators of a chunk.
+#include <algorithm>
+#include <cassert>
+
+#include "core.hpp"
+
+namespace dmrg {
+
+void Block::drop_kind(int kind) {
+    for (auto it = ops.begin(); it != ops.end();)
+        if ((int)(it->first >> 24) == kind) it = ops.erase(it);
+        else ++it;
+}
+
+std::unique_ptr<Block> empty_block(char side, int k, const MPS& mps) {
+    const int b = side == 'L' ? 0 : k;
+    return std::unique_ptr<Block>(new Block(side, b, k, mps.bonds[b], 'N'));
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// temporaries on X: complementary two-index operators touching the dot (N mode only) and the one-index
+// combinations U, V that enter the growth of S_P
+// ---------------------------------------------------------------------------------------------------------------
+void make_temps(const Ham& ham, Block& X, const Dot& dot, const std::vector<int>& far, Engine& eng) {
+    const std::vector<int> Xin = X.inside();
+    if (Xin.empty()) return;
+    std::vector<int> pool = dot.so;
+    pool.insert(pool.end(), far.begin(), far.end());
+    std::sort(pool.begin(), pool.end());
+    std::vector<LinSpec> specs;
+    auto same_shift = [](const Label& x, const Label& y) {
+        int a, b, c, d;
+        op_shift(x, a, b); op_shift(y, c, d);
+        return a == c && b == d;
+    };
+    if (X.mode == 'N') {
+        for (size_t a = 0; a < pool.size(); ++a)
+            for (size_t b = a + 1; b < pool.size(); ++b) {
+                const int P = pool[a], Q = pool[b];
+                if (!dot.has(P) && !dot.has(Q)) continue;
+                LinSpec s; s.dst = L2(K_Pt, P, Q);             // (P_PQ)^T = -sum_{R<S} w_PQRS A_RS
+                for (size_t i = 0; i < Xin.size(); ++i)
+                    for (size_t j = i + 1; j < Xin.size(); ++j) {
+                        const Label src = L2(K_A, Xin[i], Xin[j]);
+                        if (same_shift(src, s.dst)) s.items.push_back({-ham.w(P, Q, Xin[i], Xin[j]), src});
+                    }
+                specs.push_back(s);
+            }
+        for (int P : pool)
+            for (int S : pool) {
+                if (!dot.has(P) && !dot.has(S)) continue;
+                LinSpec s; s.dst = L2(K_Q, P, S);              // Q_PS = sum_{QR} w_PQRS B_QR
+                for (int Q : Xin)
+                    for (int R : Xin) {
+                        const Label src = L2(K_B, Q, R);
+                        if (same_shift(src, s.dst)) s.items.push_back({ham.w(P, Q, R, S), src});
+                    }
+                specs.push_back(s);
+            }
+    }
+    for (int P : far) {
+        for (size_t a = 0; a < dot.so.size(); ++a)
+            for (size_t b = a + 1; b < dot.so.size(); ++b) {
+                const int R = dot.so[a], S = dot.so[b];
+                LinSpec s; s.dst = L3(K_U, P, R, S);           // U_{P;RS} = sum_Q w_PQRS a+_Q
+                for (int Q : Xin) { const double w = ham.w(P, Q, R, S); if (w != 0.0) s.items.push_back({w, L1(K_C, Q)}); }
+                if (!s.items.empty()) specs.push_back(s);
+            }
+        for (int Q : dot.so)
+            for (int R : dot.so) {
+                LinSpec s; s.dst = L3(K_V, P, Q, R);           // V_{P;QR} = sum_S w_PQRS a+_S
+                for (int S : Xin) { const double w = ham.w(P, Q, R, S); if (w != 0.0) s.items.push_back({w, L1(K_C, S)}); }
+                if (!s.items.empty()) specs.push_back(s);
+            }
+    }
+    std::vector<Label> labels;
+    for (const LinSpec& s : specs) labels.push_back(s.dst);
+    X.allocate(labels, true);
+    lincomb(X, specs, false, eng);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// rotation of a list of enlarged-operator expressions into the new basis
+// ---------------------------------------------------------------------------------------------------------------
+struct NewOp { Label label; Expr expr; };
+
+static void rotate_batch(Block& X, const Dot& dot, const SiteTensor& tensor, Block& nb, const std::vector<NewOp>& list,
+                         bool temp, Engine& eng) {
+    std::vector<Label> labels;
+    for (const NewOp& o : list) labels.push_back(o.label);
+    nb.allocate(labels, temp);
+    const bool left = X.side == 'L';
+    const char* chain = left ? "Ld" : "dR";
+    const int nnew = (int)nb.basis.size();
+    const int64_t cap = eng.t_capacity();
+    DevVec<double> tmp;
+    tmp.alloc((size_t)cap);
+    GemmBatch p1, p2;
+    int64_t used = 0;
+    auto flush = [&]() {
+        run_once(p1, eng);
+        run_once(p2, eng);
+        used = 0;
+    };
+    // new-basis sector reached from X-sector i by adding (left) / removing (right) site state s
+    auto new_sector = [&](int i, int s) {
+        const Sector& q = X.basis[i];
+        return left ? find_sector(nb.basis, q.n + SITE_QN[s], q.s + SITE_QS[s])
+                    : find_sector(nb.basis, q.n - SITE_QN[s], q.s - SITE_QS[s]);
+    };
+    auto tensor_block = [&](int xsec, int s, int newsec) -> const SiteTensor::Blk* {
+        if (newsec < 0) return nullptr;
+        return left ? tensor.get(xsec, s) : tensor.get(newsec, s);
+    };
+    for (const NewOp& no : list) {
+        const OpRef& ref = nb.get(no.label);
+        const OpClass& nc = nb.classes[ref.cls];
+        std::vector<int> p2task(nnew, -1);
+        auto out_task = [&](int mi) {
+            if (p2task[mi] < 0)
+                p2task[mi] = p2.add_task(ref.ptr + nc.off[mi], pad2(nb.basis[mi].d), nb.basis[nc.out[mi]].d,
+                                         nb.basis[mi].d, 0);
+            return p2task[mi];
+        };
+        for (int mi = 0; mi < nnew; ++mi)
+            if (nc.out[mi] >= 0) out_task(mi);                 // every block is written (zero if nothing feeds it)
+        std::map<int64_t, std::pair<int, double*>> tmps;       // (o, so, mi) -> (phase-1 task, buffer)
+        for (const Term& term : no.expr) {
+            const NTerm nt = normalise(term, chain, dot);
+            const bool has_op = left ? nt.hasL : nt.hasR;
+            const Label& lab = left ? nt.L : nt.R;
+            const bool tr = left ? nt.transL : nt.transR;
+            const OpRef* op = has_op ? &X.get(lab) : nullptr;
+            const int po = has_op ? KIND_PAR[lab.kind] : 0;
+            const int pm = dot.parity(nt.dm);
+            for (int so = 0; so < 4; ++so)
+                for (int si = 0; si < 4; ++si) {
+                    const double dmv = nt.dm(so, si);
+                    if (dmv == 0.0) continue;
+                    for (int i = 0; i < (int)X.basis.size(); ++i) {
+                        OpBlockView v;
+                        int o = i;
+                        if (op) { if (!op_block(X, *op, tr, i, v)) continue; o = v.out; }
+                        const int mi = new_sector(i, si), mo = new_sector(o, so);
+                        const SiteTensor::Blk* ti = tensor_block(i, si, mi);
+                        const SiteTensor::Blk* to = tensor_block(o, so, mo);
+                        if (!ti || !to) continue;
+                        if (nc.out[mi] != mo) throw std::logic_error("rotate: quantum numbers do not close");
+                        const double sgn = left ? ((pm && (X.basis[i].n & 1)) ? -1.0 : 1.0)
+                                                : ((po && (SITE_QN[si] & 1)) ? -1.0 : 1.0);
+                        const double alpha = nt.coef * dmv * sgn;
+                        const int di = X.basis[i].d, dO = X.basis[o].d, dmi = nb.basis[mi].d;
+                        if (!op) {                             // identity block factor: straight into phase 2
+                            if (left) p2.add_seg(out_task(mi), to->ptr, to->ld, ti->ptr, ti->ld, di, SEG_TRANS_A, alpha);
+                            else      p2.add_seg(out_task(mi), to->ptr, to->ld, ti->ptr, ti->ld, di, SEG_TRANS_B, alpha);
+                            continue;
+                        }
+                        const int64_t key = ((int64_t)o * 4 + so) * nnew + mi;
+                        auto it = tmps.find(key);
+                        if (it == tmps.end()) {
+                            const int64_t sz = (int64_t)dO * pad2(dmi);
+                            if (used + sz > cap) throw Error(-3, "renormalisation workspace too small");
+                            double* buf = tmp.p + used;
+                            used += sz;
+                            const int t1 = p1.add_task(buf, pad2(dmi), dO, dmi, 0);
+                            it = tmps.emplace(key, std::make_pair(t1, buf)).first;
+                            // phase 2: out[mo <- mi] += to^T tmp (left) / to tmp (right)
+                            if (left) p2.add_seg(out_task(mi), to->ptr, to->ld, buf, pad2(dmi), dO, SEG_TRANS_A, 1.0);
+                            else      p2.add_seg(out_task(mi), to->ptr, to->ld, buf, pad2(dmi), dO, 0, 1.0);
+                        }
+                        int fl = v.trans ? SEG_TRANS_A : 0;
+                        if (!left) fl |= SEG_TRANS_B;          // ti stored [d_m x d_i]
+                        p1.add_seg(it->second.first, v.ptr, v.ld, ti->ptr, ti->ld, di, fl, alpha);
+                    }
+                }
+        }
+        if (used > cap / 2) flush();
+    }
+    flush();
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// one blocking step
+// ---------------------------------------------------------------------------------------------------------------
+static bool same_shift(const Label& x, const Label& y) {
+    int a, b, c, d;
+    op_shift(x, a, b); op_shift(y, c, d);
+    return a == c && b == d;
+}
+static Expr single(const Factor& f) { Term t; t.f.push_back(f); return Expr{t}; }
+
+std::unique_ptr<Block> grow(Block& X, const Ham& ham, const MPS& mps, char new_mode, Engine& eng) {
+    const bool left = X.side == 'L';
+    const int p = left ? X.b : X.b - 1, nbond = left ? X.b + 1 : X.b - 1;
+    const SiteTensor& tensor = mps.sites[p];
+    Dot dot(&ham, std::vector<int>{p});
+    std::unique_ptr<Block> nbp(new Block(X.side, nbond, X.k, mps.bonds[nbond], new_mode));
+    Block& nb = *nbp;
+    const std::vector<int> inside = nb.inside(), outside = nb.outside();
+    make_temps(ham, X, dot, outside, eng);
+    Gen gen(ham, block_info(X), dot);
+    std::vector<NewOp> list;
+    list.push_back({L0(K_H), gen.H()});
+    for (int P : inside) list.push_back({L1(K_C, P), gen.cre(P)});
+    for (int P : outside) {
+        Expr e;
+        for (const Term& t : gen.S(P)) e.push_back(adjoint(t));
+        list.push_back({L1(K_St, P), e});
+    }
+    if (X.mode == 'N') {
+        std::vector<NewOp> two;
+        for (size_t a = 0; a < inside.size(); ++a) {
+            for (size_t b = a + 1; b < inside.size(); ++b) two.push_back({L2(K_A, inside[a], inside[b]), gen.A(inside[a], inside[b])});
+            for (int S : inside) two.push_back({L2(K_B, inside[a], S), gen.B(inside[a], S)});
+        }
+        if (new_mode == 'N') {
+            list.insert(list.end(), two.begin(), two.end());
+            rotate_batch(X, dot, tensor, nb, list, false, eng);
+        } else {                                               // grow the normal operators, then convert
+            rotate_batch(X, dot, tensor, nb, list, false, eng);
+            rotate_batch(X, dot, tensor, nb, two, true, eng);
+            std::vector<LinSpec> specs;
+            for (size_t a = 0; a < outside.size(); ++a) {
+                for (size_t b = a + 1; b < outside.size(); ++b) {
+                    LinSpec s; s.dst = L2(K_Pt, outside[a], outside[b]);
+                    for (size_t i = 0; i < inside.size(); ++i)
+                        for (size_t j = i + 1; j < inside.size(); ++j) {
+                            const Label src = L2(K_A, inside[i], inside[j]);
+                            if (same_shift(src, s.dst)) s.items.push_back({-ham.w(outside[a], outside[b], inside[i], inside[j]), src});
+                        }
+                    specs.push_back(s);
+                }
+                for (int S : outside) {
+                    LinSpec s; s.dst = L2(K_Q, outside[a], S);
+                    for (int Q : inside)
+                        for (int R : inside) {
+                            const Label src = L2(K_B, Q, R);
+                            if (same_shift(src, s.dst)) s.items.push_back({ham.w(outside[a], Q, R, S), src});
+                        }
+                    specs.push_back(s);
+                }
+            }
+            std::vector<Label> labels;
+            for (const LinSpec& s : specs) labels.push_back(s.dst);
+            nb.allocate(labels, false);
+            lincomb(nb, specs, false, eng);
+            nb.drop_temps();
+        }
+    } else {
+        if (new_mode != 'C') throw std::logic_error("grow: complementary -> normal is not supported");
+        std::vector<char> in_x(2 * X.k, 0);
+        for (int P : X.inside()) in_x[P] = 1;
+        std::vector<NewOp> mixed;                              // new normal operators with one index on the new site
+        for (size_t a = 0; a < inside.size(); ++a) {
+            for (size_t b = a + 1; b < inside.size(); ++b)
+                if (!(in_x[inside[a]] && in_x[inside[b]])) mixed.push_back({L2(K_A, inside[a], inside[b]), gen.A(inside[a], inside[b])});
+            for (int S : inside)
+                if (!(in_x[inside[a]] && in_x[S])) mixed.push_back({L2(K_B, inside[a], S), gen.B(inside[a], S)});
+        }
+        std::vector<LinSpec> specs;
+        for (size_t a = 0; a < outside.size(); ++a) {
+            for (size_t b = a + 1; b < outside.size(); ++b) {
+                const Label l = L2(K_Pt, outside[a], outside[b]);
+                list.push_back({l, single(gen.bf(l))});
+                LinSpec s; s.dst = l;
+                for (const NewOp& m : mixed)
+                    if (m.label.kind == K_A && same_shift(m.label, l))
+                        s.items.push_back({-ham.w(outside[a], outside[b], m.label.a, m.label.b), m.label});
+                specs.push_back(s);
+            }
+            for (int S : outside) {
+                const Label l = L2(K_Q, outside[a], S);
+                list.push_back({l, single(gen.bf(l))});
+                LinSpec s; s.dst = l;
+                for (const NewOp& m : mixed)
+                    if (m.label.kind == K_B && same_shift(m.label, l))
+                        s.items.push_back({ham.w(outside[a], m.label.a, m.label.b, S), m.label});
+                specs.push_back(s);
+            }
+        }
+        rotate_batch(X, dot, tensor, nb, list, false, eng);
+        rotate_batch(X, dot, tensor, nb, mixed, true, eng);
+        lincomb(nb, specs, true, eng);
+        nb.drop_temps();
+    }
+    X.drop_temps();
+    return nbp;
+}
+
+std::unique_ptr<Block> grow_normal(Block& X, const Ham& ham, const Basis& new_basis, const SiteTensor& tensor,
+                                   bool two_index, Engine& eng) {
+    const bool left = X.side == 'L';
+    const int p = left ? X.b : X.b - 1, nbond = left ? X.b + 1 : X.b - 1;
+    Dot dot(&ham, std::vector<int>{p});
+    std::unique_ptr<Block> nbp(new Block(X.side, nbond, X.k, new_basis, 'N'));
+    Gen gen(ham, block_info(X), dot);
+    const std::vector<int> inside = nbp->inside();
+    std::vector<NewOp> list;
+    for (size_t a = 0; a < inside.size(); ++a) {
+        list.push_back({L1(K_C, inside[a]), gen.cre(inside[a])});
+        if (!two_index) continue;
+        for (size_t b = a + 1; b < inside.size(); ++b) list.push_back({L2(K_A, inside[a], inside[b]), gen.A(inside[a], inside[b])});
+        for (int S : inside) list.push_back({L2(K_B, inside[a], S), gen.B(inside[a], S)});
+    }
+    rotate_batch(X, dot, tensor, *nbp, list, false, eng);
+    return nbp;
+}
+
+}  // namespace dmrg

@@ -1,0 +1,251 @@
+// H_eff at a two-site bond: term list from the bipartition identity, block maps, and the two-phase grouped-GEMM plan
+// (DESIGN.md "Algorithm" step 5 and "Kernels").
+//
+//   y[l', a'b', r'] = sum_t c_t sgn  O_L^t[l' <- l]  x[l, ab, r]  (O_R^t[r' <- r])^T  dm^t[a'b', ab]
+//
+// Phase 1 computes each distinct intermediate once: T = O_L X (shared by every term with that left factor and input
+// block) or T = X O_R^T, whichever order needs fewer flops for the (term, block) pair.  Phase 2 gives every output
+// block to one task that sums its contributions  Y += c T O_R^T  /  Y += c O_L T  as one K-concatenated GEMM: no
+// atomics, fixed summation order.  Terms are processed in chunks bounded by the intermediate buffer.
+#include <algorithm>
+#include <cassert>
+
+#include "core.hpp"
+
+namespace dmrg {
+
+void psi_layout(const Basis& bl, const Basis& br, std::vector<PsiBlock>& layout, std::vector<int>& lookup,
+                int64_t& nnz) {
+    layout.clear();
+    lookup.assign(bl.size() * 16, -1);
+    nnz = 0;
+    for (int l = 0; l < (int)bl.size(); ++l)
+        for (int ab = 0; ab < 16; ++ab) {
+            const int a = ab >> 2, b = ab & 3;
+            const int r = find_sector(br, bl[l].n + SITE_QN[a] + SITE_QN[b], bl[l].s + SITE_QS[a] + SITE_QS[b]);
+            if (r < 0) continue;
+            lookup[l * 16 + ab] = (int)layout.size();
+            layout.push_back({l, ab, r, bl[l].d, br[r].d, nnz});
+            nnz += (int64_t)bl[l].d * br[r].d;
+        }
+}
+
+static std::vector<NTerm> heff_terms(const Ham& ham, Block& LB, Block& RB, const Dot& dot, Block*& Xout, Engine& eng) {
+    Block* X = (LB.mode == 'N') ? &LB : &RB;
+    Block* Y = (X == &LB) ? &RB : &LB;
+    if (X->mode != 'N') throw std::logic_error("heff: neither block carries normal operators");
+    if (!Y->inside().empty() && Y->mode != 'C') throw std::logic_error("heff: both blocks carry normal operators");
+    Xout = X;
+    const std::vector<int> Yin = Y->inside();
+    make_temps(ham, *X, dot, Yin, eng);
+    Gen gen(ham, block_info(*X), dot);
+    auto yf = [&](const Label& l, bool tr) {
+        Factor f; f.type = 0; f.side = Y->side; f.label = l; f.trans = tr;
+        return f;
+    };
+    std::vector<int> A = X->inside();
+    A.insert(A.end(), dot.so.begin(), dot.so.end());
+    std::sort(A.begin(), A.end());
+    Expr T = gen.H(), G;
+    if (!Yin.empty()) {
+        { Term t; t.f.push_back(yf(L0(K_H), false)); T.push_back(t); }
+        for (int P : A)                                        // a+_P^A S_P^Y
+            for (Term t : gen.cre(P)) { t.f.push_back(yf(L1(K_St, P), true)); G.push_back(t); }
+        for (int P : Yin)                                      // a+_P^Y S_P^A
+            for (const Term& s : gen.S(P)) {
+                Term t; t.coef = s.coef; t.f.push_back(yf(L1(K_C, P), false));
+                t.f.insert(t.f.end(), s.f.begin(), s.f.end());
+                G.push_back(t);
+            }
+        for (size_t a = 0; a < A.size(); ++a)                  // A_PQ^A P_PQ^Y
+            for (size_t b = a + 1; b < A.size(); ++b)
+                for (Term t : gen.A(A[a], A[b])) { t.f.push_back(yf(L2(K_Pt, A[a], A[b]), true)); G.push_back(t); }
+    }
+    for (const Term& t : G) T.push_back(t);
+    for (const Term& t : G) T.push_back(adjoint(t));
+    if (!Yin.empty())
+        for (int P : A)                                        // B_PS^A Q_PS^Y
+            for (int S : A)
+                for (Term t : gen.B(P, S)) { t.f.push_back(yf(L2(K_Q, P, S), false)); T.push_back(t); }
+    std::vector<NTerm> out;
+    out.reserve(T.size());
+    for (const Term& t : T) out.push_back(normalise(t, "LdR", dot));
+    return out;
+}
+
+int64_t Engine::t_capacity() const {
+    if (opt.workspace_bytes > 0) return opt.workspace_bytes / 8;
+    size_t free_b = 0, total_b = 0;
+    if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) return (int64_t)1 << 27;
+    int64_t cap = (int64_t)(free_b / 8) / 4;                   // a quarter of what is free ...
+    const int64_t hi = (int64_t)3 << 30;                       // ... at most 24 GiB
+    const int64_t lo = (int64_t)1 << 24;
+    return std::max(lo, std::min(cap, hi));
+}
+
+std::unique_ptr<HeffPlan> build_heff(const Ham& ham, Block& LB, Block& RB, int i, Engine& eng) {
+    std::unique_ptr<HeffPlan> pp(new HeffPlan());
+    HeffPlan& p = *pp;
+    p.bond = i;
+    psi_layout(LB.basis, RB.basis, p.layout, p.lookup, p.nnz);
+    Dot dot(&ham, std::vector<int>{i, i + 1});
+    const std::vector<NTerm> terms = heff_terms(ham, LB, RB, dot, p.X, eng);
+    p.nterms = (int64_t)terms.size();
+    p.xbuf.alloc((size_t)p.nnz);
+    p.ybuf.alloc((size_t)p.nnz);
+    const int nblk = (int)p.layout.size();
+
+    // ---- enumerate contributions term by term, chunked by the intermediate buffer ---------------------------------
+    const int64_t cap = eng.t_capacity();
+    int64_t t_max = 0;
+    struct ChunkBuild { GemmBatch p1, p2; std::vector<int> task_of; };
+    std::vector<ChunkBuild> builds;
+    std::vector<std::vector<DiagItem>> diag(nblk);
+    std::unordered_map<uint64_t, char> touched;                // operator blocks referenced (for b_alg)
+    double b_ops = 0.0;
+    auto new_chunk = [&]() {
+        builds.emplace_back();
+        ChunkBuild& cb = builds.back();
+        cb.task_of.assign(nblk, -1);
+        if (builds.size() == 1)                                // the first chunk initialises every output block
+            for (int b = 0; b < nblk; ++b)
+                cb.task_of[b] = cb.p2.add_task(p.ybuf.p + p.layout[b].off, p.layout[b].cols, p.layout[b].rows,
+                                               p.layout[b].cols, 0);
+    };
+    new_chunk();
+    int64_t used = 0;
+    std::unordered_map<uint64_t, int64_t> tcache;              // (side, op, trans, in block) -> offset into T
+    // T is allocated after planning (its size is only known then): record where its offsets must be patched in
+    struct Patch { int chunk; size_t index; int64_t off; };
+    std::vector<Patch> patchA, patchB, patchC;                 // p2 seg A / p2 seg B / p1 task C
+
+    for (size_t ti = 0; ti < terms.size(); ++ti) {
+        const NTerm& nt = terms[ti];
+        const OpRef* opL = nt.hasL ? &LB.get(nt.L) : nullptr;
+        const OpRef* opR = nt.hasR ? &RB.get(nt.R) : nullptr;
+        const int pd = dot.parity(nt.dm), pr = nt.hasR ? KIND_PAR[nt.R.kind] : 0;
+        if (used > cap / 2) { new_chunk(); used = 0; tcache.clear(); }
+        ChunkBuild& cb = builds.back();
+        const int chunk = (int)builds.size() - 1;
+        for (int bi = 0; bi < nblk; ++bi) {
+            const PsiBlock& in = p.layout[bi];
+            OpBlockView vl, vr;
+            int lo = in.l, ro = in.r;
+            if (opL) { if (!op_block(LB, *opL, nt.transL, in.l, vl)) continue; lo = vl.out; }
+            if (opR) { if (!op_block(RB, *opR, nt.transR, in.r, vr)) continue; ro = vr.out; }
+            const int nl = LB.basis[in.l].n;
+            const double sgn = ((pd * nl + pr * (nl + dot.qn[in.ab])) & 1) ? -1.0 : 1.0;
+            for (int abo = 0; abo < 16; ++abo) {
+                const double dmv = nt.dm(abo, in.ab);
+                if (dmv == 0.0) continue;
+                const int bo = p.lookup[lo * 16 + abo];
+                if (bo < 0 || p.layout[bo].r != ro) continue;
+                const PsiBlock& out = p.layout[bo];
+                const double c = nt.coef * dmv * sgn;
+                const double dl = in.rows, dr = in.cols, dlo = out.rows, dro = out.cols;
+                if (cb.task_of[bo] < 0)
+                    cb.task_of[bo] = cb.p2.add_task(p.ybuf.p + out.off, out.cols, out.rows, out.cols, TASK_ACCUM);
+                const int t2 = cb.task_of[bo];
+                const double* xin = p.xbuf.p + in.off;
+                if (opL && opR && bo == bi)
+                    diag[bi].push_back({vl.ptr, vl.ld, vr.ptr, vr.ld, c});
+                else if (opL && !opR && bo == bi) diag[bi].push_back({vl.ptr, vl.ld, nullptr, 0, c});
+                else if (!opL && opR && bo == bi) diag[bi].push_back({nullptr, 0, vr.ptr, vr.ld, c});
+                else if (!opL && !opR && bo == bi) diag[bi].push_back({nullptr, 0, nullptr, 0, c});
+                if (opL) { uint64_t k = ((uint64_t)(uintptr_t)vl.ptr); if (!touched.count(k)) { touched[k] = 1; b_ops += 8.0 * dlo * dl; } }
+                if (opR) { uint64_t k = ((uint64_t)(uintptr_t)vr.ptr); if (!touched.count(k)) { touched[k] = 1; b_ops += 8.0 * dro * dr; } }
+                if (!opL && !opR) {                            // c * X
+                    cb.p2.add_seg(t2, xin, in.cols, nullptr, 0, 0, SEG_IDENT_B, c);
+                    continue;
+                }
+                if (!opL) {                                    // Y += c X O_R^T
+                    cb.p2.add_seg(t2, xin, in.cols, vr.ptr, vr.ld, in.cols, vr.trans ? 0 : SEG_TRANS_B, c);
+                    p.f_alg += 2.0 * dl * dr * dro; p.ngemm += 1;
+                    continue;
+                }
+                if (!opR) {                                    // Y += c O_L X
+                    cb.p2.add_seg(t2, vl.ptr, vl.ld, xin, in.cols, in.rows, vl.trans ? SEG_TRANS_A : 0, c);
+                    p.f_alg += 2.0 * dlo * dl * dr; p.ngemm += 1;
+                    continue;
+                }
+                const double cost_l = 2.0 * dlo * dl * dr + 2.0 * dlo * dr * dro;   // (O_L X) O_R^T
+                const double cost_r = 2.0 * dl * dr * dro + 2.0 * dlo * dl * dro;   // O_L (X O_R^T)
+                p.f_alg += std::min(cost_l, cost_r);
+                const bool lfirst = cost_l <= cost_r;
+                const OpBlockView& v1 = lfirst ? vl : vr;
+                const uint64_t key = ((uint64_t)(uintptr_t)v1.ptr) * 2 + (lfirst ? 0 : 1);
+                const uint64_t key2 = key * 1315423911ull + (uint64_t)bi * 2654435761ull;
+                auto it = tcache.find(key2);
+                const int trows = lfirst ? out.rows : in.rows, tcols = lfirst ? in.cols : out.cols;
+                const int tld = pad2(tcols);
+                if (it == tcache.end()) {
+                    const int64_t toff = used;
+                    used += (int64_t)trows * tld;
+                    t_max = std::max(t_max, used);
+                    const int t1 = cb.p1.add_task(nullptr, tld, trows, tcols, 0);
+                    patchC.push_back({chunk, (size_t)t1, toff});
+                    if (lfirst) cb.p1.add_seg(t1, vl.ptr, vl.ld, xin, in.cols, in.rows, vl.trans ? SEG_TRANS_A : 0, 1.0);
+                    else        cb.p1.add_seg(t1, xin, in.cols, vr.ptr, vr.ld, in.cols, vr.trans ? 0 : SEG_TRANS_B, 1.0);
+                    p.ngemm += 1;
+                    it = tcache.emplace(key2, toff).first;
+                }
+                const int64_t toff = it->second;
+                if (lfirst) {                                  // Y += c T O_R^T
+                    cb.p2.add_seg(t2, nullptr, tld, vr.ptr, vr.ld, in.cols, vr.trans ? 0 : SEG_TRANS_B, c);
+                    patchA.push_back({chunk, cb.p2.segs.size() - 1, toff});
+                } else {                                       // Y += c O_L T
+                    cb.p2.add_seg(t2, vl.ptr, vl.ld, nullptr, tld, in.rows, vl.trans ? SEG_TRANS_A : 0, c);
+                    patchB.push_back({chunk, cb.p2.segs.size() - 1, toff});
+                }
+                p.ngemm += 1;
+            }
+        }
+    }
+    // ---- materialise: allocate T, patch offsets into addresses, upload ------------------------------------------------
+    p.T.alloc((size_t)std::max<int64_t>(t_max, 2));
+    for (auto& pc : patchC) builds[pc.chunk].p1.tasks[pc.index].C = p.T.p + pc.off;
+    for (auto& pa : patchA) builds[pa.chunk].p2.segs[pa.index].A = p.T.p + pa.off;
+    for (auto& pb : patchB) builds[pb.chunk].p2.segs[pb.index].B = p.T.p + pb.off;
+    p.chunks.resize(builds.size());
+    for (size_t c = 0; c < builds.size(); ++c) {
+        p.f_exec += builds[c].p1.flops + builds[c].p2.flops;
+        finalize(builds[c].p1, p.chunks[c].p1, eng);
+        finalize(builds[c].p2, p.chunks[c].p2, eng);
+    }
+    p.b_alg = b_ops + 16.0 * (double)p.nnz;
+    // ---- diagonal items -----------------------------------------------------------------------------------------------
+    std::vector<DiagItem> items;
+    std::vector<int> ptr(nblk + 1, 0), rows(nblk), cols(nblk);
+    std::vector<int64_t> offs(nblk);
+    for (int b = 0; b < nblk; ++b) {
+        items.insert(items.end(), diag[b].begin(), diag[b].end());
+        ptr[b + 1] = (int)items.size();
+        rows[b] = p.layout[b].rows; cols[b] = p.layout[b].cols; offs[b] = p.layout[b].off;
+    }
+    p.diag_items.upload(items, eng.stream);
+    p.diag_ptr.upload(ptr, eng.stream);
+    p.blk_rows.upload(rows, eng.stream);
+    p.blk_cols.upload(cols, eng.stream);
+    p.blk_off.upload(offs, eng.stream);
+    cuda_check(cudaStreamSynchronize(eng.stream), "heff plan upload");
+    return pp;
+}
+
+void heff_apply(HeffPlan& p, const double* x_dev, double* y_dev, Engine& eng) {
+    if (x_dev != p.xbuf.p)
+        cuda_check(cudaMemcpyAsync(p.xbuf.p, x_dev, (size_t)p.nnz * 8, cudaMemcpyDeviceToDevice, eng.stream), "x copy");
+    for (auto& c : p.chunks) {
+        run(c.p1, eng);
+        run(c.p2, eng);
+    }
+    if (y_dev != p.ybuf.p)
+        cuda_check(cudaMemcpyAsync(y_dev, p.ybuf.p, (size_t)p.nnz * 8, cudaMemcpyDeviceToDevice, eng.stream), "y copy");
+}
+
+void heff_diag(HeffPlan& p, double* d_dev, Engine& eng) {
+    launch_heff_diag(d_dev, (int)p.layout.size(), p.blk_off.p, p.blk_rows.p, p.blk_cols.p, p.diag_ptr.p,
+                     p.diag_items.p, eng.stream);
+    eng.launches++;
+}
+
+}  // namespace dmrg

@@ -1,0 +1,81 @@
+// Launchers of the sm_100a CUDA kernels (the only place tensor arithmetic happens).  Implemented in seg_gemm.cu,
+// vec_kernels.cu and linalg.cu.  All pointers are device pointers unless a name ends in _host.
+#pragma once
+#include <cuda_runtime_api.h>
+
+#include <cstdint>
+
+namespace dmrg {
+
+// ---- grouped, K-segmented FP64 GEMM on the FP64 tensor pipe (DMMA.8x8x4) -------------------------------------------
+//   C_task[M x N] (+)= sum_{seg in task} alpha_seg * op(A_seg)[M x K_seg] * op(B_seg)[K_seg x N]
+// One CTA owns one output tile of one task and walks the task's segment list (ownership by output tile: no
+// atomics, deterministic summation order).  This single kernel executes every dense contraction of the path:
+// H_eff psi (phase 1: T = O_L X or X O_R^T; phase 2: Y += sum_t c_t T_t O_R^T / O_L T_t, K-concatenated over
+// terms), operator renormalisation, the integral-weighted linear combinations of operator stacks, the two-site
+// tensor products and the RDM contractions.
+enum : int { SEG_TRANS_A = 1,   // A stored [K x M] row-major (used transposed)
+             SEG_TRANS_B = 2,   // B stored [N x K] row-major (used transposed); otherwise [K x N] row-major
+             SEG_IDENT_B = 4 }; // B = identity: C += alpha * A, A stored [M x N] row-major
+enum : int { TASK_ACCUM = 1 };  // C += ... instead of C = ...
+
+struct Seg {
+    const double* A;
+    const double* B;
+    int lda, ldb;
+    int K;
+    int flags;
+    double alpha;
+};
+struct Task {
+    double* C;
+    int ldc, M, N;
+    int seg_begin, seg_count;
+    int flags;
+};
+struct Tile {
+    int task, tm, tn;
+};
+constexpr int GEMM_BM = 64, GEMM_BN = 64, GEMM_BK = 16, GEMM_THREADS = 128, GEMM_STAGES = 4;
+
+void launch_seg_gemm(const Task* tasks, const Seg* segs, const Tile* tiles, int ntiles, cudaStream_t st);
+
+// ---- vector kernels (Davidson; HBM-bound) ---------------------------------------------------------------------------
+// out[j] = sum_i x[i] * Y[j*ldy + i], j < m  (deterministic two-stage reduction; out is a device array of m doubles)
+void launch_multi_dot(const double* x, const double* Y, int64_t ldy, int m, int64_t n, double* out, cudaStream_t st);
+constexpr int COMBINE_MAX = 32;
+// out[i] = beta * out[i] + sum_{j<m} coef_host[j] * V[j*ldv + i],  m <= COMBINE_MAX
+void launch_combine(double* out, double beta, const double* V, int64_t ldv, int m, const double* coef_host, int64_t n,
+                    cudaStream_t st);
+// t[i] = r[i] / clamp(diag[i] - theta), |denominator| floored at `floor` keeping its sign (reading S13)
+void launch_precond(const double* r, const double* diag, double theta, double floor, double* t, int64_t n,
+                    cudaStream_t st);
+void launch_scale(double a, double* x, int64_t n, cudaStream_t st);
+
+// diag(H_eff): for psi block b (rows x cols at off), d[off + i*cols + j] = sum_{items of b} c * ml[i*(ldl+1)] *
+// mr[j*(ldr+1)] with a null ml / mr standing for the identity.
+struct DiagItemK { const double* ml; int ldl; const double* mr; int ldr; double c; };
+void launch_heff_diag(double* d, int nblocks, const int64_t* blk_off, const int* blk_rows, const int* blk_cols,
+                      const int* item_ptr, const DiagItemK* items, cudaStream_t st);
+
+// ---- small dense helpers ---------------------------------------------------------------------------------------------
+// out[c*rows + r] = in[r*ld_in + c]   (out is [cols x rows] contiguous)
+void launch_transpose(const double* in, int rows, int cols, int ld_in, double* out, cudaStream_t st);
+// dst[r*ld_dst + c] = alpha * src[r*ld_src + c] * (row_scale ? row_scale[r] : 1) * (col_scale ? col_scale[c] : 1)
+void launch_copy2d(double* dst, int ld_dst, const double* src, int ld_src, int rows, int cols, double alpha,
+                   const double* row_scale, const double* col_scale, cudaStream_t st);
+// <A, B> = sum_ij A[i*lda+j] * B[i*ldb+j] for a batch of block pairs, out[t] += alpha[t] * <A_t, B_t> grouped by
+// target: used by the RDM accumulation (coalesced streaming of stored operators, warp-level reductions)
+struct DotPair { const double* A; const double* B; int rows, cols, lda, ldb; int target; double alpha; };
+void launch_block_dots(const DotPair* pairs, int npairs, double* out, cudaStream_t st);
+
+// ---- dense SVD of a row-major [m x n] matrix (cuSOLVER gesvd; library call) -----------------------
+// U [m x r], S [r], Vt [r x n] row-major, r = min(m, n); A is destroyed.  work: opaque per-engine handle.
+struct SvdWork;
+SvdWork* svd_create(cudaStream_t st);
+void svd_destroy(SvdWork* w);
+void svd_rowmajor(SvdWork* w, double* A, int m, int n, double* U, double* S, double* Vt, cudaStream_t st);
+// thin QR of a row-major [m x n] matrix with m >= n: Q [m x n] (orthonormal columns), R [n x n] upper triangular
+void qr_rowmajor(SvdWork* w, double* A, int m, int n, double* Q, double* R, cudaStream_t st);
+
+}  // namespace dmrg
