@@ -1,4 +1,5 @@
 // C ABI of include/dmrg_b200.h: argument checking, host<->device marshalling, exception -> status translation.
+#include <algorithm>
 #include <cmath>
 #include <cstring>
 
@@ -232,7 +233,7 @@ int dmrg_prepare_bond(dmrg_ctx* ctx, int i) {
     API_BEGIN(ctx)
     if (!eng.have_mps) return fail(eng, DMRG_ESTATE, "prepare_bond: import an MPS first");
     if (i < 0 || i > eng.k - 2) return fail(eng, DMRG_EINVAL, "prepare_bond: bond out of range");
-    eng.sweep_ready = false;
+    if (eng.sweep_ready) eng.invalidate();                     // left blocks of a finished sweep are stale
     eng.prepare_bond(i);
     return DMRG_OK;
     API_END
@@ -312,6 +313,92 @@ int dmrg_heff_stats(dmrg_ctx* ctx, int i, double* f_alg, double* f_exec, double*
     if (ngemm) *ngemm = p.ngemm;
     return DMRG_OK;
     API_END
+}
+
+int dmrg_sweep(dmrg_ctx* ctx, int D, dmrg_sweep_result* result, dmrg_bond_record* records) {
+    API_BEGIN(ctx)
+    if (!eng.have_mps) return fail(eng, DMRG_ESTATE, "sweep: import an MPS first");
+    if (D < 1) return fail(eng, DMRG_EINVAL, "sweep: D < 1");
+    if (eng.k < 2) return fail(eng, DMRG_EINVAL, "sweep: needs at least two sites");
+    if (!eng.sweep_ready)
+        for (int p = 0; p < eng.k; ++p)
+            if (eng.mps.sites[p].gauge == 'L') return fail(eng, DMRG_ESTATE, "sweep: the MPS must be right-canonical");
+    std::vector<BondRecord> recs;
+    double seconds = 0.0;
+    int warnings = 0;
+    try {
+        warnings = sweep(eng, D, recs, seconds);
+    } catch (...) {
+        eng.invalidate();                                      // a half-finished sweep leaves no usable environments
+        throw;
+    }
+    if (result) {
+        result->energy_last = recs.back().energy;
+        result->energy_min = recs[0].energy;
+        for (const BondRecord& r : recs) result->energy_min = std::min(result->energy_min, r.energy);
+        result->seconds = seconds;
+        result->n_records = (int32_t)recs.size();
+        result->warnings = warnings;
+    }
+    if (records)
+        for (size_t j = 0; j < recs.size(); ++j) {
+            const BondRecord& r = recs[j];
+            dmrg_bond_record& o = records[j];
+            o.bond = r.bond; o.forward = r.forward; o.energy = r.energy; o.residual = r.residual; o.trunc_err = r.trunc_err;
+            o.n_matvec = r.n_matvec; o.kept = r.kept; o.nsectors = r.nsectors; o.converged = r.converged; o.nnz = r.nnz;
+            o.f_alg = r.f_alg; o.seconds = r.seconds; o.seconds_matvec = r.seconds_matvec;
+        }
+    return warnings ? DMRG_ENOCONV : DMRG_OK;
+    API_END
+}
+
+int dmrg_rdm12(dmrg_ctx* ctx, double* gamma, double* Gamma, int where, void* cuda_stream) {
+    API_BEGIN(ctx)
+    (void)cuda_stream;
+    if (!eng.have_mps) return fail(eng, DMRG_ESTATE, "rdm12: import an MPS first");
+    if (!gamma) return fail(eng, DMRG_EINVAL, "rdm12: null gamma");
+    const size_t k = (size_t)eng.k;
+    if (where == DMRG_HOST) {
+        rdm12(eng, gamma, Gamma);
+    } else if (where == DMRG_DEVICE) {
+        std::vector<double> g(k * k), G(Gamma ? k * k * k * k : 0);
+        rdm12(eng, g.data(), Gamma ? G.data() : nullptr);
+        cuda_check(cudaMemcpy(gamma, g.data(), g.size() * 8, cudaMemcpyHostToDevice), "gamma upload");
+        if (Gamma) cuda_check(cudaMemcpy(Gamma, G.data(), G.size() * 8, cudaMemcpyHostToDevice), "Gamma upload");
+    } else return fail(eng, DMRG_EINVAL, "rdm12: bad `where`");
+    return DMRG_OK;
+    API_END
+}
+
+int dmrg_rdm_stats(dmrg_ctx* ctx, double* seconds, double* bytes_streamed, double* flops) {
+    API_BEGIN(ctx)
+    if (seconds) *seconds = eng.rdm_seconds;
+    if (bytes_streamed) *bytes_streamed = eng.rdm_bytes;
+    if (flops) *flops = eng.rdm_flops;
+    return DMRG_OK;
+    API_END
+}
+
+int dmrg_grouped_gemm(int ntasks, const int64_t* c_ptr, const int32_t* ldc, const int32_t* m, const int32_t* n,
+                      const int32_t* seg_begin, const int32_t* seg_count, const int32_t* task_flags, int nsegs,
+                      const int64_t* a_ptr, const int64_t* b_ptr, const int32_t* lda, const int32_t* ldb,
+                      const int32_t* kk, const int32_t* seg_flags, const double* alpha, void* cuda_stream) {
+    if (ntasks < 0 || nsegs < 0) return DMRG_EINVAL;
+    try {
+        Engine tmp;                                            // only the stream and the launch counter are used
+        tmp.stream = (cudaStream_t)cuda_stream;
+        GemmBatch b;
+        for (int t = 0; t < ntasks; ++t) {
+            if (seg_begin[t] < 0 || seg_count[t] < 0 || seg_begin[t] + seg_count[t] > nsegs) return DMRG_EINVAL;
+            b.add_task((double*)(uintptr_t)c_ptr[t], ldc[t], m[t], n[t], task_flags[t]);
+            for (int s = seg_begin[t]; s < seg_begin[t] + seg_count[t]; ++s)
+                b.add_seg(t, (const double*)(uintptr_t)a_ptr[s], lda[s], (const double*)(uintptr_t)b_ptr[s], ldb[s], kk[s],
+                          seg_flags[s], alpha[s]);
+        }
+        run_once(b, tmp);
+    } catch (const Error& e) { return e.code; }
+    catch (...) { return DMRG_ECUDA; }
+    return DMRG_OK;
 }
 
 }  // extern "C"

@@ -75,7 +75,5 @@ struct SvdWork;
 SvdWork* svd_create(cudaStream_t st);
 void svd_destroy(SvdWork* w);
 void svd_rowmajor(SvdWork* w, double* A, int m, int n, double* U, double* S, double* Vt, cudaStream_t st);
-// thin QR of a row-major [m x n] matrix with m >= n: Q [m x n] (orthonormal columns), R [n x n] upper triangular
-void qr_rowmajor(SvdWork* w, double* A, int m, int n, double* Q, double* R, cudaStream_t st);
 
 }  // namespace dmrg

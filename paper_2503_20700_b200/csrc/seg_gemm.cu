@@ -1,4 +1,4 @@
-// Grouped, K-segmented FP64 GEMM for sm_100a: see seg_gemm.cuh.
+// Grouped, K-segmented FP64 GEMM for sm_100a: see kernels.hpp.
 //
 // Pipeline: cp.async (LDGSTS, 16-byte, zero-filling ragged edges) -> 4-stage shared-memory ring -> register
 // fragments -> DMMA.8x8x4 (mma.sync.aligned.m8n8k4.f64).  sm_100a has no FP64 kind in tcgen05/UMMA, so the warp-
@@ -240,7 +240,7 @@ __global__ void __launch_bounds__(NT) seg_gemm_kernel(const Task* __restrict__ t
 
 }  // namespace
 
-void launch_seg_gemm(const Task* d_tasks, const Seg* d_segs, const Tile* d_tiles, int ntiles, void* stream) {
+void launch_seg_gemm(const Task* d_tasks, const Seg* d_segs, const Tile* d_tiles, int ntiles, cudaStream_t stream) {
     if (ntiles <= 0) return;
     static bool configured = false;
     const int smem_bytes = ST * STAGE_DOUBLES * (int)sizeof(double);
@@ -248,7 +248,7 @@ void launch_seg_gemm(const Task* d_tasks, const Seg* d_segs, const Tile* d_tiles
         cudaFuncSetAttribute(seg_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
         configured = true;
     }
-    seg_gemm_kernel<<<ntiles, NT, smem_bytes, (cudaStream_t)stream>>>(d_tasks, d_segs, d_tiles, ntiles);
+    seg_gemm_kernel<<<ntiles, NT, smem_bytes, stream>>>(d_tasks, d_segs, d_tiles, ntiles);
 }
 
 }  // namespace dmrg

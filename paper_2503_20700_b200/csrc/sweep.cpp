@@ -1,0 +1,339 @@
+// Davidson driver, decomposition + truncation, and the two-site sweep (DESIGN.md
+// "Algorithm" step 4 and readings S12-S18).  Vectors live on the device; the host sees O(subspace) scalars per
+// iteration and the singular values of each bond.
+#include <algorithm>
+#include <chrono>
+#include <cmath>
+
+#include "core.hpp"
+
+namespace dmrg {
+
+// ---------------------------------------------------------------------------------------------------------------
+// tiny symmetric eigenproblem of the Rayleigh-Ritz step (host, cyclic Jacobi; m <= 32)
+// ---------------------------------------------------------------------------------------------------------------
+static void jacobi_eigh(std::vector<double> a, int m, std::vector<double>& w, std::vector<double>& v) {
+    v.assign((size_t)m * m, 0.0);
+    for (int i = 0; i < m; ++i) v[(size_t)i * m + i] = 1.0;
+    for (int sweep = 0; sweep < 100; ++sweep) {
+        double off = 0.0, diag = 0.0;
+        for (int i = 0; i < m; ++i)
+            for (int j = 0; j < m; ++j) (i == j ? diag : off) += a[(size_t)i * m + j] * a[(size_t)i * m + j];
+        if (off <= 1e-32 * (diag + off) || off == 0.0) break;
+        for (int p = 0; p < m; ++p)
+            for (int q = p + 1; q < m; ++q) {
+                const double apq = a[(size_t)p * m + q];
+                if (apq == 0.0) continue;
+                const double zeta = (a[(size_t)q * m + q] - a[(size_t)p * m + p]) / (2.0 * apq);
+                const double t = (zeta >= 0 ? 1.0 : -1.0) / (std::fabs(zeta) + std::sqrt(1.0 + zeta * zeta));
+                const double c = 1.0 / std::sqrt(1.0 + t * t), s = c * t;
+                for (int r = 0; r < m; ++r) {
+                    const double x = a[(size_t)r * m + p], y = a[(size_t)r * m + q];
+                    a[(size_t)r * m + p] = c * x - s * y; a[(size_t)r * m + q] = s * x + c * y;
+                }
+                for (int r = 0; r < m; ++r) {
+                    const double x = a[(size_t)p * m + r], y = a[(size_t)q * m + r];
+                    a[(size_t)p * m + r] = c * x - s * y; a[(size_t)q * m + r] = s * x + c * y;
+                }
+                for (int r = 0; r < m; ++r) {
+                    const double x = v[(size_t)r * m + p], y = v[(size_t)r * m + q];
+                    v[(size_t)r * m + p] = c * x - s * y; v[(size_t)r * m + q] = s * x + c * y;
+                }
+            }
+    }
+    w.resize(m);
+    for (int i = 0; i < m; ++i) w[i] = a[(size_t)i * m + i];
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Davidson (reading S13): single root, diagonal preconditioner, twice-applied Gram-Schmidt, restart
+// ---------------------------------------------------------------------------------------------------------------
+DavidsonResult davidson(HeffPlan& p, double* x_dev, Engine& eng) {
+    const int64_t n = p.nnz;
+    const int maxsub = eng.opt.davidson_max_subspace;
+    cudaStream_t st = eng.stream;
+    DevVec<double> V, W, diag, r, scal;
+    V.alloc((size_t)maxsub * n); W.alloc((size_t)maxsub * n); diag.alloc((size_t)n); r.alloc((size_t)n);
+    scal.alloc(COMBINE_MAX + 2);
+    std::vector<double> hs((size_t)COMBINE_MAX + 2);
+    auto dots = [&](const double* x, const double* Y, int m) {          // -> hs[0..m)
+        launch_multi_dot(x, Y, n, m, n, scal.p, st);
+        eng.launches += 2;
+        cuda_check(cudaMemcpyAsync(hs.data(), scal.p, sizeof(double) * m, cudaMemcpyDeviceToHost, st), "dots");
+        cuda_check(cudaStreamSynchronize(st), "dots");
+    };
+    cudaEvent_t e0, e1;
+    cuda_check(cudaEventCreate(&e0), "event"); cuda_check(cudaEventCreate(&e1), "event");
+    double ms_matvec = 0.0;
+    auto matvec = [&](const double* v, double* w) {
+        cuda_check(cudaEventRecord(e0, st), "event");
+        heff_apply(p, v, w, eng);
+        cuda_check(cudaEventRecord(e1, st), "event");
+        cuda_check(cudaEventSynchronize(e1), "event");
+        float ms = 0.f;
+        cuda_check(cudaEventElapsedTime(&ms, e0, e1), "event");
+        ms_matvec += ms;
+    };
+    heff_diag(p, diag.p, eng);
+    dots(x_dev, x_dev, 1);
+    if (!(hs[0] > 0.0)) throw Error(-2, "davidson: zero initial guess");
+    cuda_check(cudaMemcpyAsync(V.p, x_dev, (size_t)n * 8, cudaMemcpyDeviceToDevice, st), "copy");
+    launch_scale(1.0 / std::sqrt(hs[0]), V.p, n, st); eng.launches++;
+    matvec(V.p, W.p);
+    int m = 1, nmv = 1;
+    std::vector<double> H((size_t)maxsub * maxsub, 0.0);
+    dots(W.p, V.p, 1);
+    H[0] = hs[0];
+    DavidsonResult res{0.0, 1e300, 0, false, 0.0};
+    std::vector<double> w, s, coef(COMBINE_MAX);
+    for (int iter = 0; iter < eng.opt.davidson_max_iter; ++iter) {
+        std::vector<double> hm((size_t)m * m);
+        for (int i = 0; i < m; ++i)
+            for (int j = 0; j < m; ++j) hm[(size_t)i * m + j] = H[(size_t)i * maxsub + j];
+        jacobi_eigh(hm, m, w, s);
+        int lo = 0;
+        for (int i = 1; i < m; ++i) if (w[i] < w[lo]) lo = i;
+        const double theta = w[lo];
+        for (int i = 0; i < m; ++i) coef[i] = s[(size_t)i * m + lo];
+        // r = sum s_i W_i - theta sum s_i V_i
+        launch_combine(r.p, 0.0, W.p, n, m, coef.data(), n, st);
+        std::vector<double> c2(m);
+        for (int i = 0; i < m; ++i) c2[i] = -theta * coef[i];
+        launch_combine(r.p, 1.0, V.p, n, m, c2.data(), n, st);
+        eng.launches += 2;
+        dots(r.p, r.p, 1);
+        const double rn = std::sqrt(hs[0]);
+        res.theta = theta; res.residual = rn; res.n_matvec = nmv;
+        const bool done = rn <= eng.opt.davidson_tol;
+        if (done || iter + 1 == eng.opt.davidson_max_iter) {
+            res.converged = done;
+            launch_combine(x_dev, 0.0, V.p, n, m, coef.data(), n, st); eng.launches++;
+            dots(x_dev, x_dev, 1);
+            launch_scale(1.0 / std::sqrt(hs[0]), x_dev, n, st); eng.launches++;
+            break;
+        }
+        // preconditioned correction (into r)
+        launch_precond(r.p, diag.p, theta, 1e-8, r.p, n, st); eng.launches++;
+        if (m >= maxsub) {                                                  // restart with the Ritz pair
+            DevVec<double> u, hu;
+            u.alloc((size_t)n); hu.alloc((size_t)n);
+            launch_combine(u.p, 0.0, V.p, n, m, coef.data(), n, st);
+            launch_combine(hu.p, 0.0, W.p, n, m, coef.data(), n, st);
+            eng.launches += 2;
+            dots(u.p, u.p, 1);
+            const double inv = 1.0 / std::sqrt(hs[0]);
+            launch_scale(inv, u.p, n, st); launch_scale(inv, hu.p, n, st); eng.launches += 2;
+            cuda_check(cudaMemcpyAsync(V.p, u.p, (size_t)n * 8, cudaMemcpyDeviceToDevice, st), "copy");
+            cuda_check(cudaMemcpyAsync(W.p, hu.p, (size_t)n * 8, cudaMemcpyDeviceToDevice, st), "copy");
+            cuda_check(cudaStreamSynchronize(st), "restart");
+            m = 1;
+            dots(W.p, V.p, 1);
+            H[0] = hs[0];
+        }
+        for (int gs = 0; gs < 2; ++gs) {                                    // t -= V (V^T t), twice
+            dots(r.p, V.p, m);
+            std::vector<double> c(m);
+            for (int i = 0; i < m; ++i) c[i] = -hs[i];
+            launch_combine(r.p, 1.0, V.p, n, m, c.data(), n, st); eng.launches++;
+        }
+        dots(r.p, r.p, 1);
+        const double nt = std::sqrt(hs[0]);
+        if (nt < 1e-14) {                                                   // subspace exhausted
+            launch_combine(x_dev, 0.0, V.p, n, m, coef.data(), n, st); eng.launches++;
+            dots(x_dev, x_dev, 1);
+            launch_scale(1.0 / std::sqrt(hs[0]), x_dev, n, st); eng.launches++;
+            break;
+        }
+        double* vnew = V.p + (size_t)m * n;
+        double* wnew = W.p + (size_t)m * n;
+        cuda_check(cudaMemcpyAsync(vnew, r.p, (size_t)n * 8, cudaMemcpyDeviceToDevice, st), "copy");
+        launch_scale(1.0 / nt, vnew, n, st); eng.launches++;
+        matvec(vnew, wnew);
+        ++nmv;
+        dots(wnew, V.p, m + 1);                                             // new column of V^T W
+        for (int i = 0; i <= m; ++i) { H[(size_t)i * maxsub + m] = hs[i]; H[(size_t)m * maxsub + i] = hs[i]; }
+        ++m;
+    }
+    cuda_check(cudaStreamSynchronize(st), "davidson");
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    res.n_matvec = nmv;
+    res.seconds_matvec = ms_matvec * 1e-3;
+    return res;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// theta[l, a, b, r] = sum_m T_i[(l,a)][:, m] T_{i+1}[(m,b)][m, :]      (prediction of the next guess, reading S16)
+// ---------------------------------------------------------------------------------------------------------------
+void two_site_tensor(const MPS& mps, int i, const HeffPlan& p, double* theta_dev, Engine& eng) {
+    GemmBatch b;
+    const SiteTensor& ta = mps.sites[i];
+    const SiteTensor& tb = mps.sites[i + 1];
+    for (const PsiBlock& blk : p.layout) {
+        const int t = b.add_task(theta_dev + blk.off, blk.cols, blk.rows, blk.cols, 0);
+        const SiteTensor::Blk* x = ta.get(blk.l, blk.ab >> 2);
+        if (!x) continue;
+        const SiteTensor::Blk* y = tb.get(x->r, blk.ab & 3);
+        if (!y) continue;
+        b.add_seg(t, x->ptr, x->ld, y->ptr, y->ld, x->cols, 0, 1.0);
+    }
+    run_once(b, eng);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// SVD per enlarged-left sector and global top-D selection that never cuts a near-degenerate cluster (reading S14)
+// ---------------------------------------------------------------------------------------------------------------
+void split_theta(MPS& mps, int i, const HeffPlan& p, const double* theta, int D, bool forward, Engine& eng,
+                 double& trunc_err, int& kept, int& nsectors) {
+    cudaStream_t st = eng.stream;
+    const Basis& bl = mps.bonds[i];
+    const Basis& br = mps.bonds[i + 2];
+    struct Sec {
+        int n, s;
+        std::vector<std::pair<int, int>> rows, cols;          // (l, a) and (b, r)
+        std::vector<int> roff, coff;
+        int nr = 0, nc = 0, rk = 0;
+        DevVec<double> M, U, S, Vt;
+        std::vector<double> sv;
+        int keep = 0;
+    };
+    std::map<std::pair<int, int>, Sec> secs;
+    for (const PsiBlock& b : p.layout) {
+        const int a = b.ab >> 2, bb = b.ab & 3;
+        const auto q = std::make_pair(bl[b.l].n + SITE_QN[a], bl[b.l].s + SITE_QS[a]);
+        Sec& sc = secs[q];
+        sc.n = q.first; sc.s = q.second;
+        if (std::find(sc.rows.begin(), sc.rows.end(), std::make_pair(b.l, a)) == sc.rows.end()) sc.rows.push_back({b.l, a});
+        if (std::find(sc.cols.begin(), sc.cols.end(), std::make_pair(bb, b.r)) == sc.cols.end()) sc.cols.push_back({bb, b.r});
+    }
+    // norm of theta (the kept state is rescaled to unit norm afterwards)
+    DevVec<double> scal;
+    scal.alloc(1);
+    launch_multi_dot(theta, theta, p.nnz, 1, p.nnz, scal.p, st); eng.launches += 2;
+    double nrm2 = 0.0;
+    cuda_check(cudaMemcpyAsync(&nrm2, scal.p, 8, cudaMemcpyDeviceToHost, st), "norm");
+    cuda_check(cudaStreamSynchronize(st), "norm");
+    const double inv_nrm = 1.0 / std::sqrt(nrm2);
+    struct PoolItem { double sv; int sec, j; };
+    std::vector<PoolItem> pool;
+    std::vector<Sec*> order;
+    for (auto& kv : secs) {                                    // std::map iterates in ascending (n, s)
+        Sec& sc = kv.second;
+        std::sort(sc.rows.begin(), sc.rows.end());
+        std::sort(sc.cols.begin(), sc.cols.end());
+        for (auto& rc : sc.rows) { sc.roff.push_back(sc.nr); sc.nr += bl[rc.first].d; }
+        for (auto& cc : sc.cols) { sc.coff.push_back(sc.nc); sc.nc += br[cc.second].d; }
+        sc.rk = std::min(sc.nr, sc.nc);
+        sc.M.alloc((size_t)sc.nr * sc.nc);
+        cuda_check(cudaMemsetAsync(sc.M.p, 0, (size_t)sc.nr * sc.nc * 8, st), "memset");
+        for (size_t ri = 0; ri < sc.rows.size(); ++ri)
+            for (size_t ci = 0; ci < sc.cols.size(); ++ci) {
+                const int idx = p.lookup[sc.rows[ri].first * 16 + sc.rows[ri].second * 4 + sc.cols[ci].first];
+                if (idx < 0 || p.layout[idx].r != sc.cols[ci].second) continue;
+                const PsiBlock& b = p.layout[idx];
+                launch_copy2d(sc.M.p + (size_t)sc.roff[ri] * sc.nc + sc.coff[ci], sc.nc, theta + b.off, b.cols, b.rows,
+                              b.cols, inv_nrm, nullptr, nullptr, st);
+                eng.launches++;
+            }
+        sc.U.alloc((size_t)sc.nr * sc.rk); sc.S.alloc((size_t)sc.rk); sc.Vt.alloc((size_t)sc.rk * sc.nc);
+        svd_rowmajor(eng.svd, sc.M.p, sc.nr, sc.nc, sc.U.p, sc.S.p, sc.Vt.p, st);
+        sc.sv.resize(sc.rk);
+        cuda_check(cudaMemcpyAsync(sc.sv.data(), sc.S.p, (size_t)sc.rk * 8, cudaMemcpyDeviceToHost, st), "sv");
+        cuda_check(cudaStreamSynchronize(st), "sv");
+        for (int j = 0; j < sc.rk; ++j) pool.push_back({sc.sv[j], (int)order.size(), j});
+        order.push_back(&sc);
+    }
+    std::vector<int> idx(pool.size());
+    for (size_t t = 0; t < idx.size(); ++t) idx[t] = (int)t;
+    std::stable_sort(idx.begin(), idx.end(), [&](int x, int y) { return pool[x].sv > pool[y].sv; });
+    int count = 0;
+    for (int t : idx) if (pool[t].sv > eng.opt.sv_floor) ++count;
+    int m = std::min(D, count);
+    const int m0 = m;
+    while (m > 0 && m < count && pool[idx[m]].sv >= (1.0 - eng.opt.cluster_rel_gap) * pool[idx[m - 1]].sv) --m;
+    if (m == 0) m = m0;
+    if (m == 0) throw Error(-2, "split: the two-site state has no singular value above the floor");
+    double kept_w = 0.0;
+    for (int t = 0; t < m; ++t) { kept_w += pool[idx[t]].sv * pool[idx[t]].sv; order[pool[idx[t]].sec]->keep++; }
+    trunc_err = std::max(0.0, 1.0 - kept_w);
+    const double scale = 1.0 / std::sqrt(kept_w);
+    kept = m;
+    Basis mid;
+    for (Sec* sc : order) if (sc->keep > 0) mid.push_back({sc->n, sc->s, sc->keep});
+    nsectors = (int)mid.size();
+    // new site tensors
+    SiteTensor A, B;
+    make_site_tensor(A, bl, mid);
+    make_site_tensor(B, mid, br);
+    if (A.nnz) cuda_check(cudaMemsetAsync(A.data.p, 0, (size_t)A.nnz * 8, st), "memset");
+    if (B.nnz) cuda_check(cudaMemsetAsync(B.data.p, 0, (size_t)B.nnz * 8, st), "memset");
+    for (Sec* sc : order) {
+        if (sc->keep == 0) continue;
+        const int mi = find_sector(mid, sc->n, sc->s);
+        const int nk = sc->keep;
+        for (size_t ri = 0; ri < sc->rows.size(); ++ri) {
+            const SiteTensor::Blk* blk = A.get(sc->rows[ri].first, sc->rows[ri].second);
+            if (!blk || blk->r != mi) throw std::logic_error("split: A block missing");
+            launch_copy2d(blk->ptr, blk->ld, sc->U.p + (size_t)sc->roff[ri] * sc->rk, sc->rk, blk->rows, nk,
+                          forward ? 1.0 : scale, nullptr, forward ? nullptr : sc->S.p, st);
+            eng.launches++;
+        }
+        for (size_t ci = 0; ci < sc->cols.size(); ++ci) {
+            const SiteTensor::Blk* blk = B.get(mi, sc->cols[ci].first);
+            if (!blk || blk->r != sc->cols[ci].second) throw std::logic_error("split: B block missing");
+            launch_copy2d(blk->ptr, blk->ld, sc->Vt.p + sc->coff[ci], sc->nc, nk, blk->cols, forward ? scale : 1.0,
+                          forward ? sc->S.p : nullptr, nullptr, st);
+            eng.launches++;
+        }
+    }
+    cuda_check(cudaStreamSynchronize(st), "split");
+    A.gauge = forward ? 'L' : 'C';
+    B.gauge = forward ? 'C' : 'R';
+    mps.bonds[i + 1] = mid;
+    mps.sites[i] = std::move(A);
+    mps.sites[i + 1] = std::move(B);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// one sweep: forward pass over bonds 0..k-2, backward pass k-2..0 (reading S12)
+// ---------------------------------------------------------------------------------------------------------------
+static BondRecord optimise(Engine& eng, int i, int D, bool forward) {
+    const auto t0 = std::chrono::steady_clock::now();
+    eng.plan.reset();
+    eng.plan = build_heff(eng.ham, *eng.L.at(i), *eng.R.at(i + 2), i, eng);
+    HeffPlan& p = *eng.plan;
+    DevVec<double> theta;
+    theta.alloc((size_t)p.nnz);
+    two_site_tensor(eng.mps, i, p, theta.p, eng);
+    const DavidsonResult dr = davidson(p, theta.p, eng);
+    BondRecord rec;
+    rec.bond = i; rec.forward = forward ? 1 : 0;
+    rec.energy = dr.theta; rec.residual = dr.residual; rec.n_matvec = dr.n_matvec; rec.converged = dr.converged ? 1 : 0;
+    rec.nnz = p.nnz; rec.f_alg = p.f_alg; rec.seconds_matvec = dr.seconds_matvec;
+    split_theta(eng.mps, i, p, theta.p, D, forward, eng, rec.trunc_err, rec.kept, rec.nsectors);
+    eng.plan.reset();                                          // releases the temporaries before the block grows
+    if (forward) eng.L[i + 1] = grow(*eng.L.at(i), eng.ham, eng.mps, eng.mode_L(i + 1), eng);
+    else         eng.R[i + 1] = grow(*eng.R.at(i + 2), eng.ham, eng.mps, eng.mode_R(i + 1), eng);
+    rec.seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+    return rec;
+}
+
+int sweep(Engine& eng, int D, std::vector<BondRecord>& recs, double& seconds) {
+    const auto t0 = std::chrono::steady_clock::now();
+    const int k = eng.k;
+    if (!eng.sweep_ready) {
+        eng.invalidate();
+        eng.keep_env_stack = true;
+        eng.L[0] = empty_block('L', k, eng.mps);
+        eng.ensure_right(2);
+        eng.sweep_ready = true;
+    }
+    recs.clear();
+    for (int i = 0; i <= k - 2; ++i) recs.push_back(optimise(eng, i, D, true));
+    for (int i = k - 2; i >= 0; --i) recs.push_back(optimise(eng, i, D, false));
+    seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+    int warnings = 0;
+    for (const BondRecord& r : recs) if (!r.converged) ++warnings;
+    return warnings;
+}
+
+}  // namespace dmrg
