@@ -1,0 +1,363 @@
+#!/usr/bin/env python
+"""bench.py - measures BASELINE.json's metric on one B200 (or N independent replicas).
+
+Metric: H_eff psi FP64 TFLOP/s at the mid-chain two-site bond (reading S22) of BASELINE config 4 (circumcoronene
+CAS(54,54) PPP, D = 4096) on a seeded synthetic MPS with that block structure; a "step" is one H_eff psi.
+  value      device-resident x, y (torch CUDA tensors), CUDA events on the launching stream, F_exec / t
+  e2e        the same call through the C ABI with HOST buffers (pinned x uploaded, y read back, inside the timer)
+  roofline   the grouped FP64 DMMA GEMM kernel (the only kernel of H_eff psi) against the FP64 tensor peak
+  cpu_baseline  the CPU oracle, as it stands, timed on a bounded sample of the same workload class
+  extras     seconds per sweep and 1-/2-RDM time on a small config (--extras), bond-step breakdown
+`--impl reference` times the oracle (the reference arm of this tier).  Inputs are synthetic and seeded
+(synth/); nothing here reads /root/reference.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "heff_psi_fp64_tflops_midchain"
+UNIT = "TFLOP/s"
+FP64_FLOP_PER_CLK_SM = 128.0          # DMMA: 64 FP64 FMA / clk / SM
+N_SM = 148
+BF16_NOMINAL_TF = 2250.0
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="BASELINE config 1..5 (default 4: the metric's workload)")
+    ap.add_argument("--D", type=int, default=0, help="bond dimension override (0 = the config's)")
+    ap.add_argument("--bond", type=int, default=-1, help="two-site bond (default mid-chain k/2-1)")
+    ap.add_argument("--extras", type=int, default=1, help="1: also time a small sweep + RDM (config 1)")
+    ap.add_argument("--cpu-baseline", type=int, default=1)
+    ap.add_argument("--sample-config", type=int, default=2, help="config of the oracle's bounded sample")
+    ap.add_argument("--sample-D", type=int, default=96)
+    return ap.parse_args()
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm=d["hbm_gbs"], bf16=d["bf16_tflops"], bf16_sus=d.get("bf16_tflops_sustained", d["bf16_tflops"]),
+                    sm_max=d.get("sm_max_mhz", 1965.0), src="measured")
+    return dict(hbm=6650.0, bf16=1590.0, bf16_sus=1400.0, sm_max=1965.0, src="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thr = threading.Thread(target=self._read, daemon=True)
+            self.thr.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[1])), mx.append(float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[4:8]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None,
+                    reasons=sorted(reasons), samples=len(sm))
+
+
+def build_workload(cfg_id, D, bond):
+    """Hamiltonian of BASELINE config cfg_id and a seeded random block-sparse MPS, left-orthonormal on sites < i and
+    right-orthonormal on sites >= i (H_eff at bond i needs nothing else)."""
+    from synth import make_config, random_mps, mps_to_blob_arrays
+    cfg = make_config(cfg_id)
+    k = cfg["k"]
+    D = D or cfg["D"]
+    i = bond if bond >= 0 else k // 2 - 1
+    mps = random_mps(k, cfg["n_elec"], 0, D, seed=cfg["seed"] + 1000, gauge="LR:%d" % i)
+    return cfg, D, i, mps, mps_to_blob_arrays(mps)
+
+
+def oracle_sample(args, steps, warmup):
+    """The oracle, as it stands, on a bounded sample: H_eff psi at the mid-chain bond of the sample config at a reduced
+    bond dimension (its own environments built by its own renormalisation, untimed).  Returns (TFLOP/s, info)."""
+    from oracle import dmrg as odmrg
+    cfg, D, i, mps, _ = build_workload(args.sample_config, args.sample_D, -1)
+    oham = odmrg.Ham(cfg["h"], cfg["eri"])
+    t0 = time.perf_counter()
+    oL = odmrg.build_left(mps, oham, i)[-1]
+    oR = odmrg.build_right(mps, oham, i + 2)[i + 2]
+    H = odmrg.Heff(oL, oR, oham, i)
+    t_env = time.perf_counter() - t0
+    x = np.random.default_rng(1).normal(size=H.nnz)
+    x /= np.linalg.norm(x)
+    f_alg = oracle_falg(H)
+    for _ in range(warmup):
+        H.apply(x)
+    ts = []
+    for _ in range(steps):
+        t0 = time.perf_counter()
+        H.apply(x)
+        ts.append(time.perf_counter() - t0)
+    sec = float(np.mean(ts))
+    try:
+        import threadpoolctl
+        cores = max([p.get("num_threads", 1) for p in threadpoolctl.threadpool_info()] or [1])
+    except Exception:
+        cores = os.cpu_count()
+    info = dict(kind="oracle", cores=int(cores), host_cores=os.cpu_count(),
+                sample="%s, D=%d, two-site bond %d, nnz=%d, %d H_eff psi applications of oracle/dmrg.py (environment "
+                       "build %.1f s untimed); flops = the oracle's own per-block GEMM count" %
+                       (cfg["name"], D, i, H.nnz, steps, t_env), ms_per_step=sec * 1e3, f_alg=f_alg)
+    return f_alg / sec / 1e12, info
+
+
+def oracle_falg(H):
+    """Flops of the matrix products one oracle H_eff psi executes, counted by walking the oracle's own term list with
+    the loop structure of oracle.dmrg.Heff.apply_blocks: (ml @ x) @ mr^T per (term, site-state pair, block), twice
+    for terms that add their Hermitian conjugate.  Integer bookkeeping only - no oracle arithmetic is re-done."""
+    f = 0.0
+    for (coef, E, F, hc) in H.terms:
+        for (ao, ai), OL in E.grid.items():
+            for (bo, bi), OR in F.grid.items():
+                for li, (lo, ml) in OL.blocks.items():
+                    kin = (li, ai, bi)
+                    if kin not in H.by_key:
+                        continue
+                    ri, m_in, n_in = H.by_key[kin]
+                    if ri not in OR.blocks:
+                        continue
+                    ro, mr = OR.blocks[ri]
+                    if (lo, ao, bo) not in H.by_key:
+                        continue
+                    m_out, n_out = ml.shape[0], mr.shape[0]
+                    g = 2.0 * m_out * m_in * n_in + 2.0 * m_out * n_in * n_out
+                    f += g
+                    if hc:
+                        f += 2.0 * m_in * m_out * n_out + 2.0 * m_in * n_out * n_in
+    return f
+
+
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def run_reference(args):
+    """Reference arm of this tier = the CPU oracle on the box's host cores; rank 0 only."""
+    rank, _, _ = dist_env()
+    if rank != 0:
+        return
+    val, info = oracle_sample(args, args.steps, args.warmup)
+    cfg_name = "BASELINE config %d" % args.config
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": info["ms_per_step"], "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg_name + " (bounded sample: see cpu_baseline.sample)"},
+            "cpu_baseline": dict(info, value=val, unit=UNIT),
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def time_small_extras(P, torch):
+    """Seconds per sweep and 1-/2-RDM time on BASELINE config 1 (D = 64): the remaining rows of the hot path
+    (a1, a3, a4, a5, a6) exercised end to end in the same run."""
+    from synth import make_config, random_mps, mps_to_blob_arrays
+    out = {}
+    cfg = make_config(1)
+    k, n = cfg["k"], cfg["n_elec"]
+    mps = random_mps(k, n, 0, 64, seed=cfg["seed"] + 1000, gauge="R")
+    ctx = P.dmrg_create(k, n, 0, cfg["h"], cfg["eri"])
+    try:
+        P.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, 0)
+        secs, e = [], None
+        for _ in range(3):
+            r = P.dmrg_sweep(ctx, 64, k)
+            secs.append(r["seconds"])
+            e = r["energy_last"]
+        out["sweep"] = {"workload": cfg["name"] + " D=64", "s_per_sweep": secs, "energy_last_eh": e + cfg["e_core"],
+                        "matvecs_last_sweep": int(sum(b["n_matvec"] for b in r["bonds"]))}
+        try:
+            t0 = time.perf_counter()
+            g, G = P.dmrg_rdm12(ctx, k, True)
+            torch.cuda.synchronize()
+            st = P.dmrg_rdm_stats(ctx)
+            out["rdm12"] = {"workload": cfg["name"] + " D=64", "seconds": time.perf_counter() - t0,
+                            "device_seconds": st["seconds"], "trace_gamma": float(np.trace(g)),
+                            "gbytes_streamed": st["bytes_streamed"] / 1e9}
+        except P.binding.DmrgError as ex:
+            out["rdm12"] = {"error": str(ex)}
+    finally:
+        P.dmrg_destroy(ctx)
+    return out
+
+
+def run_ours(args):
+    import torch
+    import __graft_entry__ as entry
+    rank, local_rank, world = dist_env()
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    torch.cuda.set_device(local_rank)
+    if rank == 0:
+        entry.build()
+    if world > 1:
+        dist.barrier()
+    import paper_2503_20700_b200 as P
+    peaks = measured_peaks()
+    dev = torch.device("cuda", local_rank)
+
+    # ---- workload: every rank an independent replica of the same seeded problem ("replicas only") -----------------
+    t_setup = time.perf_counter()
+    cfg, D, i, mps, blob = build_workload(args.config, args.D, args.bond)
+    k, n = cfg["k"], cfg["n_elec"]
+    ctx = P.dmrg_create(k, n, 0, cfg["h"], cfg["eri"], keep_env_stack=0, device_id=local_rank)
+    P.dmrg_mps_import(ctx, blob, k, n, 0)
+    t_env = time.perf_counter()
+    P.dmrg_prepare_bond(ctx, i)                      # renormalisation of both environments + block maps (a1, a5)
+    torch.cuda.synchronize()
+    t_env = time.perf_counter() - t_env
+    nnz, layout = P.dmrg_heff_layout(ctx, i)
+    st = P.dmrg_heff_stats(ctx, i)
+    g = torch.Generator(device="cpu").manual_seed(1234 + rank)
+    xh = torch.randn(nnz, dtype=torch.float64, generator=g)
+    xh /= xh.norm()
+    x = xh.to(dev)
+    y = torch.empty_like(x)
+    t_setup = time.perf_counter() - t_setup
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    # ---- device-resident timing ---------------------------------------------------------------------------------
+    for _ in range(max(args.warmup, 3)):
+        P.dmrg_heff_apply(ctx, i, x, y)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    l0 = P.dmrg_launch_count(ctx)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    ev[0].record()
+    for s in range(args.steps):
+        P.dmrg_heff_apply(ctx, i, x, y)
+        ev[s + 1].record()
+    barrier()
+    clocks = sampler.stop()
+    launches = P.dmrg_launch_count(ctx) - l0
+    per_step = [ev[s].elapsed_time(ev[s + 1]) for s in range(args.steps)]
+    total_ms = ev[0].elapsed_time(ev[-1])
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = world * st["f_exec"] / (ms_per_step * 1e-3) / 1e12
+
+    # ---- end to end: host buffers through the C ABI (H2D of x and D2H of y inside the timer) -----------------------
+    xp = xh.pin_memory().numpy()
+    yp = torch.empty(nnz, dtype=torch.float64).pin_memory().numpy()
+    P.dmrg_heff_apply(ctx, i, xp, yp)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        P.dmrg_heff_apply(ctx, i, xp, yp)
+    torch.cuda.synchronize()
+    e2e_s = (time.perf_counter() - t0) / args.steps
+    if world > 1:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e = world * st["f_exec"] / e2e_s / 1e12
+    y_check = float(np.linalg.norm(yp))
+    assert np.isfinite(y_check) and y_check > 0.0
+    dev_bytes = P.dmrg_device_bytes(ctx)
+    P.dmrg_destroy(ctx)
+    if rank != 0:
+        return
+
+    # ---- roofline of the dominant kernel (seg_gemm_kernel: every launch of H_eff psi is this kernel) ---------------
+    nominal = N_SM * FP64_FLOP_PER_CLK_SM * peaks["sm_max"] * 1e6 / 1e12
+    peak = peaks["bf16"] * nominal / BF16_NOMINAL_TF
+    t_flop = st["f_exec"] / (peak * 1e12)
+    t_byte = st["b_alg"] / (peaks["hbm"] * 1e9)
+    achieved = st["f_exec"] / (ms_per_step * 1e-3) / 1e12
+    roof = {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+            "traffic": None, "kernel": "seg_gemm_kernel (FP64 DMMA.8x8x4)", "launches_per_step": launches / args.steps,
+            "peak_source": "%s bf16 burst %.1f TF x nominal FP64/bf16 ratio (%.1f / %.0f TF); FP64 nominal = 148 SM x "
+                           "128 flop/clk x %.0f MHz" % (peaks["src"], peaks["bf16"], nominal, BF16_NOMINAL_TF, peaks["sm_max"]),
+            "peak_nominal_fp64": nominal, "frac_of_nominal": achieved / nominal,
+            "f_alg": st["f_alg"], "f_exec": st["f_exec"], "b_alg": st["b_alg"],
+            "roofline_ms": max(t_flop, t_byte) * 1e3, "hbm_ms": t_byte * 1e3}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "%s, D=%d, H_eff psi at two-site bond %d (mid-chain), seeded random block-sparse MPS; "
+                                   "replicas only for N>1" % (cfg["name"], D, i),
+                       "nnz_psi": nnz, "psi_blocks": len(layout), "terms": st["nterms"], "gemms": st["ngemm"],
+                       "l2": "inputs larger than L2 (operator blocks %.1f GB)" % ((st["b_alg"] - 16.0 * nnz) / 1e9),
+                       "device_gb": dev_bytes / 1e9, "env_build_s": t_env, "setup_s": t_setup},
+            "ms_per_step_minmax": [min(per_step), max(per_step)],
+            "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 8 * nnz, "d2h_bytes_per_step": 8 * nnz,
+                    "ms_per_step": e2e_s * 1e3},
+            "gpu_launches": int(launches), "clocks": clocks, "roofline": roof}
+    if args.extras:
+        line["extras"] = time_small_extras(P, torch)
+    if args.cpu_baseline and world == 1:
+        v, info = oracle_sample(args, 3, 1)
+        line["cpu_baseline"] = dict(info, value=v, unit=UNIT)
+    print(json.dumps(line))
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+    if int(os.environ.get("WORLD_SIZE", 1)) > 1:
+        import torch.distributed as dist
+        if dist.is_initialized():
+            dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,70 @@
+"""Parity of the device two-site sweep (Davidson + SVD truncation + fused renormalisation) with the CPU oracle on
+the same imported MPS.  Tolerance (BASELINE.json north_star): sweep energies <= 1e-8 Eh; parity runs use the
+Davidson tolerance 1e-10 of reading S13 so the converged eigenpair does not depend on the iteration path."""
+import numpy as np
+import pytest
+
+from oracle import dmrg as odmrg
+from oracle import fci as ofci
+from synth import random_dense, random_mps, mps_to_blob_arrays, make_config
+
+pytestmark = pytest.mark.gpu
+TOL_E = 1e-8
+
+
+def _run_both(lib, h, eri, k, n, s2, D, nsweeps, seed, Dinit=None):
+    mps = random_mps(k, n, s2, Dinit or D, seed=seed, gauge="R")
+    ctx = lib.dmrg_create(k, n, s2, h, eri, davidson_tol=1e-10)
+    eng = odmrg.SweepEngine(h, eri, mps, davidson_tol=1e-10)
+    out = []
+    try:
+        lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, s2)
+        for _ in range(nsweeps):
+            g = lib.dmrg_sweep(ctx, D, k)
+            o = eng.sweep(D)
+            out.append((g, o))
+    finally:
+        lib.dmrg_destroy(ctx)
+    return out
+
+
+@pytest.mark.parametrize("k,n,s2,D", [(4, 4, 0, 16), (6, 6, 0, 12), (6, 7, 1, 16), (8, 8, 0, 24)])
+def test_sweep_energies_match_oracle(lib, k, n, s2, D):
+    h, eri = random_dense(k, 90 + k)
+    for (g, o) in _run_both(lib, h, eri, k, n, s2, D, 2, seed=17 + k):
+        assert abs(g["energy_last"] - o["energy_last"]) <= TOL_E
+        assert abs(g["energy_min"] - o["energy_min"]) <= TOL_E
+        for rg, ro in zip(g["bonds"], o["bonds"]):
+            assert rg["bond"] == ro["bond"] and rg["kept"] == ro["kept"] and rg["nsectors"] == ro["nsectors"]
+            assert abs(rg["energy"] - ro["energy"]) <= TOL_E
+            assert abs(rg["trunc_err"] - ro["trunc_err"]) <= 1e-9
+
+
+def test_untruncated_sweep_reaches_fci(lib):
+    """At full bond dimension the device sweep converges to the brute-force FCI ground energy."""
+    k, n, s2 = 6, 6, 0
+    h, eri = random_dense(k, 123)
+    space = ofci.FCISpace(k, n, s2)
+    e_fci = space.ground_state(h, eri)[0]
+    mps = random_mps(k, n, s2, 8, seed=5, gauge="R")
+    ctx = lib.dmrg_create(k, n, s2, h, eri, davidson_tol=1e-10)
+    try:
+        lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, s2)
+        e = None
+        for _ in range(4):
+            e = lib.dmrg_sweep(ctx, 4096, k)["energy_last"]
+        assert abs(e - e_fci) <= 1e-9
+    finally:
+        lib.dmrg_destroy(ctx)
+
+
+def test_sweep_config1_naphthalene_D64(lib):
+    """BASELINE config 1 at D=64, 4 sweeps: per-sweep energies GPU vs oracle (reading S11: D=64 is truncated)."""
+    cfg = make_config(1)
+    k, n = cfg["k"], cfg["n_elec"]
+    res = _run_both(lib, cfg["h"], cfg["eri"], k, n, 0, 64, cfg["sweeps"], seed=cfg["seed"] + 1000)
+    for (g, o) in res:
+        assert abs(g["energy_last"] - o["energy_last"]) <= TOL_E
+        assert abs(g["energy_min"] - o["energy_min"]) <= TOL_E
+    # variational: never below the FCI energy quoted in tests/golden (computed by the oracle's brute force)
+    assert res[-1][0]["energy_last"] + cfg["e_core"] >= -0.8822829988 - 1e-8
