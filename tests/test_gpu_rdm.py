@@ -1,0 +1,88 @@
+"""Parity of the device RDM pass (dmrg_rdm12) with the CPU oracle, element by element, plus the invariants of
+BASELINE.json north_star: Tr gamma = N, sum_r Gamma_pqrr = (N-1) gamma_pq, symmetries, and
+E = sum h gamma + 1/2 sum (pq|rs) Gamma.  Tolerance: RDM max-abs error <= 1e-10."""
+import numpy as np
+import pytest
+
+from oracle import dmrg as odmrg
+from oracle import fci as ofci
+from synth import random_dense, random_mps, mps_to_blob_arrays, blob_arrays_to_mps, make_config
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-10
+
+
+def _invariants(g, G, n):
+    k = g.shape[0]
+    assert abs(np.trace(g) - n) <= 1e-9
+    assert np.abs(g - g.T).max() <= 1e-10
+    assert np.abs(np.einsum("pqrr->pq", G) - (n - 1) * g).max() <= 1e-9
+    assert abs(np.einsum("pprr->", G) - n * (n - 1)) <= 1e-8
+    assert np.abs(G - G.transpose(2, 3, 0, 1)).max() <= 1e-10
+    assert np.abs(G - G.transpose(1, 0, 3, 2)).max() <= 1e-10
+    w = np.linalg.eigvalsh(g)
+    assert w.min() >= -1e-9 and w.max() <= 2 + 1e-9 and k > 0
+
+
+@pytest.mark.parametrize("k,n,s2,D", [(2, 2, 0, 4), (3, 3, 1, 6), (4, 4, 0, 8), (5, 6, 0, 12), (6, 6, 0, 16),
+                                      (6, 7, 1, 12), (6, 3, -1, 10), (8, 8, 0, 20)])
+def test_rdm12_random_mps_vs_oracle(lib, k, n, s2, D):
+    h, eri = random_dense(k, 300 + k)
+    mps = random_mps(k, n, s2, D, seed=31 + k, gauge="R")
+    for key in list(mps["tensors"][0].keys()):                      # an unnormalised centre must not matter
+        mps["tensors"][0][key] = 1.7 * mps["tensors"][0][key]
+    g0, G0 = odmrg.rdm12(h, eri, mps, True)
+    ctx = lib.dmrg_create(k, n, s2, h, eri)
+    try:
+        lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, s2)
+        g, G = lib.dmrg_rdm12(ctx, k, True)
+        g1, _ = lib.dmrg_rdm12(ctx, k, False)                       # 1-RDM only path; repeated calls allowed
+    finally:
+        lib.dmrg_destroy(ctx)
+    assert np.abs(g - g0).max() <= TOL and np.abs(G - G0).max() <= TOL and np.abs(g1 - g0).max() <= TOL
+    _invariants(g, G, n)
+
+
+def test_rdm12_after_sweep_energy_and_fci(lib):
+    """After untruncated sweeps the RDMs equal the brute-force FCI RDMs and reproduce the energy (S20)."""
+    k, n, s2 = 6, 6, 0
+    h, eri = random_dense(k, 77)
+    space = ofci.FCISpace(k, n, s2)
+    e_fci, c = space.ground_state(h, eri)
+    gf, Gf = space.rdm12(c)
+    mps = random_mps(k, n, s2, 8, seed=9, gauge="R")
+    ctx = lib.dmrg_create(k, n, s2, h, eri, davidson_tol=1e-11)
+    try:
+        lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, s2)
+        for _ in range(4):
+            e = lib.dmrg_sweep(ctx, 4096, k)["energy_last"]
+        g, G = lib.dmrg_rdm12(ctx, k, True)
+    finally:
+        lib.dmrg_destroy(ctx)
+    assert abs(e - e_fci) <= 1e-9
+    assert np.abs(g - gf).max() <= 1e-7 and np.abs(G - Gf).max() <= 1e-7     # state converged to ~1e-11 in energy
+    e_rdm = np.einsum("pq,pq->", h, g) + 0.5 * np.einsum("pqrs,pqrs->", eri, G)
+    assert abs(e_rdm - e_fci) <= 1e-9
+    _invariants(g, G, n)
+
+
+def test_rdm12_config1_truncated_sweep_vs_oracle(lib):
+    """BASELINE config 1 at D = 64: RDMs of the GPU's final MPS vs the oracle's RDM pass on that same MPS."""
+    cfg = make_config(1)
+    k, n = cfg["k"], cfg["n_elec"]
+    mps = random_mps(k, n, 0, 64, seed=cfg["seed"] + 1000, gauge="R")
+    ctx = lib.dmrg_create(k, n, 0, cfg["h"], cfg["eri"])
+    try:
+        lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, 0)
+        for _ in range(2):
+            r = lib.dmrg_sweep(ctx, 64, k)
+        g, G = lib.dmrg_rdm12(ctx, k, True)
+        arrs, n2, s2 = lib.dmrg_mps_export(ctx, k)
+    finally:
+        lib.dmrg_destroy(ctx)
+    final = blob_arrays_to_mps(k, n, 0, *arrs)
+    g0, G0 = odmrg.rdm12(cfg["h"], cfg["eri"], final, True)
+    assert np.abs(g - g0).max() <= TOL and np.abs(G - G0).max() <= TOL
+    _invariants(g, G, n)
+    e_rdm = np.einsum("pq,pq->", cfg["h"], g) + 0.5 * np.einsum("pqrs,pqrs->", cfg["eri"], G)
+    assert e_rdm >= r["energy_min"] - 1e-9                           # <Psi|H|Psi> of the truncated MPS (reading S20)
