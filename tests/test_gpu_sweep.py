@@ -68,3 +68,35 @@ def test_sweep_config1_naphthalene_D64(lib):
         assert abs(g["energy_min"] - o["energy_min"]) <= TOL_E
     # variational: never below the FCI energy quoted in tests/golden (computed by the oracle's brute force)
     assert res[-1][0]["energy_last"] + cfg["e_core"] >= -0.8822829988 - 1e-8
+
+
+def _golden():
+    import os
+    vals = {}
+    for line in open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "config1_fci.txt")):
+        if not line.startswith("#"):
+            key, rest = line.split(None, 1)
+            vals[key] = [float(x) for x in rest.split()]
+    return vals
+
+
+def test_config1_untruncated_reaches_golden_fci(lib):
+    """BASELINE config 1 with no truncation (reading S11: the exact mid-chain rank is 1024, so D >= 1024): energy vs
+    the brute-force FCI value of tests/golden/config1_fci.txt to 1e-8 Eh, natural occupations of the device 1-RDM."""
+    gold = _golden()
+    cfg = make_config(1)
+    k, n = cfg["k"], cfg["n_elec"]
+    mps = random_mps(k, n, 0, 64, seed=cfg["seed"] + 1000, gauge="R")
+    ctx = lib.dmrg_create(k, n, 0, cfg["h"], cfg["eri"], davidson_tol=1e-9)
+    try:
+        lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, 0)
+        for _ in range(5):
+            r = lib.dmrg_sweep(ctx, 2048, k)
+        g, G = lib.dmrg_rdm12(ctx, k, True)
+    finally:
+        lib.dmrg_destroy(ctx)
+    assert abs(r["energy_last"] - gold["e_el_fci"][0]) <= 1e-8
+    occ = np.sort(np.linalg.eigvalsh(g))[::-1]
+    assert np.abs(occ - np.array(gold["natural_occupations"])).max() <= 1e-6
+    e_rdm = np.einsum("pq,pq->", cfg["h"], g) + 0.5 * np.einsum("pqrs,pqrs->", cfg["eri"], G)
+    assert abs(e_rdm - gold["e_el_fci"][0]) <= 1e-8
