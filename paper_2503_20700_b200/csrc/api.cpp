@@ -1,6 +1,7 @@
 // C ABI of include/dmrg_b200.h: argument checking, host<->device marshalling, exception -> status translation.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 
 #include "../../include/dmrg_b200.h"
@@ -109,6 +110,7 @@ int dmrg_create(dmrg_ctx** out, int k, int n_elec, int two_sz, const double* h, 
         eng.ham.h.assign(h, h + (size_t)k * k);
         eng.ham.eri.assign(eri, eri + (size_t)k * k * k * k);
         eng.svd = svd_create(eng.stream);
+        { const char* g = std::getenv("DMRG_B200_GENERIC_GEMM"); eng.force_generic_gemm = g && g[0] == '1'; }
     } catch (...) {
         delete ctx;
         return DMRG_ECUDA;
@@ -387,6 +389,7 @@ int dmrg_grouped_gemm(int ntasks, const int64_t* c_ptr, const int32_t* ldc, cons
     try {
         Engine tmp;                                            // only the stream and the launch counter are used
         tmp.stream = (cudaStream_t)cuda_stream;
+        { const char* g = std::getenv("DMRG_B200_GENERIC_GEMM"); tmp.force_generic_gemm = g && g[0] == '1'; }
         GemmBatch b;
         for (int t = 0; t < ntasks; ++t) {
             if (seg_begin[t] < 0 || seg_count[t] < 0 || seg_begin[t] + seg_count[t] > nsegs) return DMRG_EINVAL;

@@ -65,7 +65,7 @@ void make_site_tensor(SiteTensor& t, const Basis& bl, const Basis& br) {
 
 int GemmBatch::add_task(double* C, int ldc, int M, int N, int flags) {
     Task t;
-    t.C = C; t.ldc = ldc; t.M = M; t.N = N; t.seg_begin = 0; t.seg_count = 0; t.flags = flags;
+    t.C = C; t.ldc = ldc; t.M = M; t.N = N; t.seg_begin = 0; t.seg_count = 0; t.flags = flags; t.ngemm = 0;
     tasks.push_back(t);
     return (int)tasks.size() - 1;
 }
@@ -87,7 +87,28 @@ void finalize(GemmBatch& b, GemmLaunch& out, Engine& eng) {
     std::vector<Seg> sorted(b.segs.size());
     std::vector<int> cursor(nt);
     for (int t = 0; t < nt; ++t) cursor[t] = b.tasks[t].seg_begin;
-    for (size_t j = 0; j < b.segs.size(); ++j) sorted[cursor[b.seg_task[j]]++] = b.segs[j];   // stable
+    // stable within a task, GEMM segments first, identity-B segments last
+    for (auto& t : b.tasks) t.ngemm = 0;
+    for (size_t j = 0; j < b.segs.size(); ++j)
+        if (!(b.segs[j].flags & SEG_IDENT_B)) sorted[cursor[b.seg_task[j]]++] = b.segs[j];
+    for (int t = 0; t < nt; ++t) b.tasks[t].ngemm = cursor[t] - b.tasks[t].seg_begin;
+    for (size_t j = 0; j < b.segs.size(); ++j)
+        if (b.segs[j].flags & SEG_IDENT_B) sorted[cursor[b.seg_task[j]]++] = b.segs[j];
+    bool aligned = true;
+    for (const Seg& sg : sorted) {
+        if (sg.flags & SEG_IDENT_B) continue;
+        if ((((uintptr_t)sg.A) & 15) || (((uintptr_t)sg.B) & 15) || (sg.lda & 1) || (sg.ldb & 1)) { aligned = false; break; }
+    }
+    // a transposed / row operand is read in pieces of pad2(extent) doubles: the leading dimension must cover them
+    for (int t = 0; t < nt && aligned; ++t)
+        for (int j = 0; j < b.tasks[t].ngemm; ++j) {
+            const Seg& sg = sorted[b.tasks[t].seg_begin + j];
+            const int M = b.tasks[t].M, N = b.tasks[t].N, K = sg.K;
+            const int needA = (sg.flags & SEG_TRANS_A) ? pad2(M) : pad2(K);
+            const int needB = (sg.flags & SEG_TRANS_B) ? pad2(K) : pad2(N);
+            if (sg.lda < needA || sg.ldb < needB) { aligned = false; break; }
+        }
+    out.aligned = aligned;
     // tiles, heaviest tasks first so that the tail of the launch is made of short tiles
     std::vector<double> weight(nt, 0.0);
     for (int t = 0; t < nt; ++t)
@@ -106,13 +127,17 @@ void finalize(GemmBatch& b, GemmLaunch& out, Engine& eng) {
     out.tasks.upload(b.tasks, eng.stream);
     out.segs.upload(sorted, eng.stream);
     out.tiles.upload(tiles, eng.stream);
+    if (!out.counter.p) out.counter.alloc(1);
     out.ntiles = (int)tiles.size();
     out.flops = b.flops;
     cuda_check(cudaStreamSynchronize(eng.stream), "descriptor upload");   // host vectors die after this call
 }
 void run(const GemmLaunch& l, Engine& eng) {
     if (l.ntiles == 0) return;
-    launch_seg_gemm(l.tasks.p, l.segs.p, l.tiles.p, l.ntiles, eng.stream);
+    if (l.aligned && !eng.force_generic_gemm)
+        launch_seg_gemm_tma(l.tasks.p, l.segs.p, l.tiles.p, l.ntiles, l.counter.p, eng.stream);
+    else
+        launch_seg_gemm(l.tasks.p, l.segs.p, l.tiles.p, l.ntiles, eng.stream);
     eng.launches++;
 }
 void run_once(GemmBatch& b, Engine& eng) {
@@ -272,17 +297,18 @@ void lincomb(Block& blk, const std::vector<LinSpec>& specs, bool accumulate, Eng
         const Stack& ss = blk.stacks[src_stack];
         if (ss.cls != ds.cls) throw std::logic_error("lincomb: class mismatch");
         const int n_src = (int)ss.members.size();
-        std::vector<double> W((size_t)n_dst * n_src, 0.0);
+        const int ldw = pad2(n_src);                           // even leading dimension: bulk-copy kernel eligible
+        std::vector<double> W((size_t)n_dst * ldw, 0.0);
         for (const LinSpec* s : kv.second) {
             const int r = blk.get(s->dst).row;
-            for (const LinItem& it : s->items) W[(size_t)r * n_src + blk.get(it.src).row] += it.coef;
+            for (const LinItem& it : s->items) W[(size_t)r * ldw + blk.get(it.src).row] += it.coef;
         }
         keep.emplace_back();
         keep.back().upload(W, eng.stream);
         cuda_check(cudaStreamSynchronize(eng.stream), "lincomb upload");
         // the row length can exceed the int range of Task::N only beyond 2^31 doubles per operator: not reachable
         const int t = batch.add_task(ds.base, (int)cls.ld, n_dst, (int)cls.nnz, accumulate ? TASK_ACCUM : 0);
-        batch.add_seg(t, keep.back().p, n_src, ss.base, (int)cls.ld, n_src, 0, 1.0);
+        batch.add_seg(t, keep.back().p, ldw, ss.base, (int)cls.ld, n_src, 0, 1.0);
     }
     run_once(batch, eng);
 }

@@ -83,7 +83,9 @@ struct GemmLaunch {                               // device-resident descriptors
     DevVec<Task> tasks;
     DevVec<Seg> segs;
     DevVec<Tile> tiles;
+    DevVec<int> counter;                          // dynamic tile counter of the persistent kernel
     int ntiles = 0;
+    bool aligned = false;                         // every GEMM operand 16-byte aligned, even ld: bulk-copy kernel
     double flops = 0.0;
 };
 struct Engine;
@@ -156,7 +158,7 @@ std::unique_ptr<Block> grow_normal(Block& X, const Ham& ham, const Basis& new_ba
 BlockInfo block_info(const Block& b);
 
 // ---- H_eff ---------------------------------------------------------------------------------------------------------
-struct PsiBlock { int l, ab, r, rows, cols; int64_t off; };
+struct PsiBlock { int l, ab, r, rows, cols; int64_t off; int64_t poff; };   // poff: offset in the padded (even ld) copy
 typedef DiagItemK DiagItem;                      // null pointer = identity factor
 struct HeffPlan {
     int bond = -1;
@@ -165,7 +167,9 @@ struct HeffPlan {
     int64_t nnz = 0;
     struct Chunk { GemmLaunch p1, p2; };
     std::vector<Chunk> chunks;
-    DevVec<double> T, xbuf, ybuf;
+    DevVec<double> T, xbuf, ybuf, xpad;           // xpad: x with even leading dimensions, 16-byte aligned blocks
+    int64_t nnz_pad = 0;
+    DevVec<int64_t> blk_poff;
     DevVec<DiagItem> diag_items;
     DevVec<int> diag_ptr;                         // per psi block range into diag_items
     DevVec<int64_t> blk_off;
@@ -211,6 +215,7 @@ struct Engine {
     double rdm_seconds = 0, rdm_bytes = 0, rdm_flops = 0;
     bool keep_env_stack = true;
     bool sweep_ready = false;                     // environments consistent with the sweep position
+    bool force_generic_gemm = false;              // DMRG_B200_GENERIC_GEMM=1: always the cp.async kernel (A/B testing)
     char mode_L(int b) const { return b <= bsw ? 'N' : 'C'; }
     char mode_R(int b) const { return b >= bsw + 3 ? 'N' : 'C'; }
     int64_t t_capacity() const;                   // doubles available for intermediates

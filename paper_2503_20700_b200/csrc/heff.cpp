@@ -25,7 +25,7 @@ void psi_layout(const Basis& bl, const Basis& br, std::vector<PsiBlock>& layout,
             const int r = find_sector(br, bl[l].n + SITE_QN[a] + SITE_QN[b], bl[l].s + SITE_QS[a] + SITE_QS[b]);
             if (r < 0) continue;
             lookup[l * 16 + ab] = (int)layout.size();
-            layout.push_back({l, ab, r, bl[l].d, br[r].d, nnz});
+            layout.push_back({l, ab, r, bl[l].d, br[r].d, nnz, 0});
             nnz += (int64_t)bl[l].d * br[r].d;
         }
 }
@@ -94,6 +94,9 @@ std::unique_ptr<HeffPlan> build_heff(const Ham& ham, Block& LB, Block& RB, int i
     p.xbuf.alloc((size_t)p.nnz);
     p.ybuf.alloc((size_t)p.nnz);
     const int nblk = (int)p.layout.size();
+    for (PsiBlock& b : p.layout) { b.poff = p.nnz_pad; p.nnz_pad += (int64_t)b.rows * pad2(b.cols); }
+    p.xpad.alloc((size_t)std::max<int64_t>(p.nnz_pad, 2));
+    cuda_check(cudaMemsetAsync(p.xpad.p, 0, (size_t)std::max<int64_t>(p.nnz_pad, 2) * 8, eng.stream), "memset");
 
     // ---- enumerate contributions term by term, chunked by the intermediate buffer ---------------------------------
     const int64_t cap = eng.t_capacity();
@@ -146,7 +149,8 @@ std::unique_ptr<HeffPlan> build_heff(const Ham& ham, Block& LB, Block& RB, int i
                 if (cb.task_of[bo] < 0)
                     cb.task_of[bo] = cb.p2.add_task(p.ybuf.p + out.off, out.cols, out.rows, out.cols, TASK_ACCUM);
                 const int t2 = cb.task_of[bo];
-                const double* xin = p.xbuf.p + in.off;
+                const double* xin = p.xpad.p + in.poff;        // padded copy of x: every GEMM operand is aligned
+                const int xld = pad2(in.cols);
                 if (opL && opR && bo == bi)
                     diag[bi].push_back({vl.ptr, vl.ld, vr.ptr, vr.ld, c});
                 else if (opL && !opR && bo == bi) diag[bi].push_back({vl.ptr, vl.ld, nullptr, 0, c});
@@ -155,16 +159,16 @@ std::unique_ptr<HeffPlan> build_heff(const Ham& ham, Block& LB, Block& RB, int i
                 if (opL) { uint64_t k = ((uint64_t)(uintptr_t)vl.ptr); if (!touched.count(k)) { touched[k] = 1; b_ops += 8.0 * dlo * dl; } }
                 if (opR) { uint64_t k = ((uint64_t)(uintptr_t)vr.ptr); if (!touched.count(k)) { touched[k] = 1; b_ops += 8.0 * dro * dr; } }
                 if (!opL && !opR) {                            // c * X
-                    cb.p2.add_seg(t2, xin, in.cols, nullptr, 0, 0, SEG_IDENT_B, c);
+                    cb.p2.add_seg(t2, xin, xld, nullptr, 0, 0, SEG_IDENT_B, c);
                     continue;
                 }
                 if (!opL) {                                    // Y += c X O_R^T
-                    cb.p2.add_seg(t2, xin, in.cols, vr.ptr, vr.ld, in.cols, vr.trans ? 0 : SEG_TRANS_B, c);
+                    cb.p2.add_seg(t2, xin, xld, vr.ptr, vr.ld, in.cols, vr.trans ? 0 : SEG_TRANS_B, c);
                     p.f_alg += 2.0 * dl * dr * dro; p.ngemm += 1;
                     continue;
                 }
                 if (!opR) {                                    // Y += c O_L X
-                    cb.p2.add_seg(t2, vl.ptr, vl.ld, xin, in.cols, in.rows, vl.trans ? SEG_TRANS_A : 0, c);
+                    cb.p2.add_seg(t2, vl.ptr, vl.ld, xin, xld, in.rows, vl.trans ? SEG_TRANS_A : 0, c);
                     p.f_alg += 2.0 * dlo * dl * dr; p.ngemm += 1;
                     continue;
                 }
@@ -184,8 +188,8 @@ std::unique_ptr<HeffPlan> build_heff(const Ham& ham, Block& LB, Block& RB, int i
                     t_max = std::max(t_max, used);
                     const int t1 = cb.p1.add_task(nullptr, tld, trows, tcols, 0);
                     patchC.push_back({chunk, (size_t)t1, toff});
-                    if (lfirst) cb.p1.add_seg(t1, vl.ptr, vl.ld, xin, in.cols, in.rows, vl.trans ? SEG_TRANS_A : 0, 1.0);
-                    else        cb.p1.add_seg(t1, xin, in.cols, vr.ptr, vr.ld, in.cols, vr.trans ? 0 : SEG_TRANS_B, 1.0);
+                    if (lfirst) cb.p1.add_seg(t1, vl.ptr, vl.ld, xin, xld, in.rows, vl.trans ? SEG_TRANS_A : 0, 1.0);
+                    else        cb.p1.add_seg(t1, xin, xld, vr.ptr, vr.ld, in.cols, vr.trans ? 0 : SEG_TRANS_B, 1.0);
                     p.ngemm += 1;
                     it = tcache.emplace(key2, toff).first;
                 }
@@ -203,6 +207,7 @@ std::unique_ptr<HeffPlan> build_heff(const Ham& ham, Block& LB, Block& RB, int i
     }
     // ---- materialise: allocate T, patch offsets into addresses, upload ------------------------------------------------
     p.T.alloc((size_t)std::max<int64_t>(t_max, 2));
+    cuda_check(cudaMemsetAsync(p.T.p, 0, (size_t)std::max<int64_t>(t_max, 2) * 8, eng.stream), "memset");   // finite pads
     for (auto& pc : patchC) builds[pc.chunk].p1.tasks[pc.index].C = p.T.p + pc.off;
     for (auto& pa : patchA) builds[pa.chunk].p2.segs[pa.index].A = p.T.p + pa.off;
     for (auto& pb : patchB) builds[pb.chunk].p2.segs[pb.index].B = p.T.p + pb.off;
@@ -222,6 +227,9 @@ std::unique_ptr<HeffPlan> build_heff(const Ham& ham, Block& LB, Block& RB, int i
         ptr[b + 1] = (int)items.size();
         rows[b] = p.layout[b].rows; cols[b] = p.layout[b].cols; offs[b] = p.layout[b].off;
     }
+    std::vector<int64_t> poffs(nblk);
+    for (int b = 0; b < nblk; ++b) poffs[b] = p.layout[b].poff;
+    p.blk_poff.upload(poffs, eng.stream);
     p.diag_items.upload(items, eng.stream);
     p.diag_ptr.upload(ptr, eng.stream);
     p.blk_rows.upload(rows, eng.stream);
@@ -232,8 +240,9 @@ std::unique_ptr<HeffPlan> build_heff(const Ham& ham, Block& LB, Block& RB, int i
 }
 
 void heff_apply(HeffPlan& p, const double* x_dev, double* y_dev, Engine& eng) {
-    if (x_dev != p.xbuf.p)
-        cuda_check(cudaMemcpyAsync(p.xbuf.p, x_dev, (size_t)p.nnz * 8, cudaMemcpyDeviceToDevice, eng.stream), "x copy");
+    // x (packed exchange layout) -> padded, aligned copy read by the GEMM kernel
+    launch_pad_blocks(p.xpad.p, x_dev, (int)p.layout.size(), p.blk_poff.p, p.blk_off.p, p.blk_rows.p, p.blk_cols.p, eng.stream);
+    eng.launches++;
     for (auto& c : p.chunks) {
         run(c.p1, eng);
         run(c.p2, eng);

@@ -32,6 +32,7 @@ struct Task {
     int ldc, M, N;
     int seg_begin, seg_count;
     int flags;
+    int ngemm;                  // segments [seg_begin, seg_begin + ngemm) are GEMM segments, the rest identity-B (set by finalize)
 };
 struct Tile {
     int task, tm, tn;
@@ -39,6 +40,9 @@ struct Tile {
 constexpr int GEMM_BM = 64, GEMM_BN = 64, GEMM_BK = 16, GEMM_THREADS = 128, GEMM_STAGES = 4;
 
 void launch_seg_gemm(const Task* tasks, const Seg* segs, const Tile* tiles, int ntiles, cudaStream_t st);
+// Same contract, bulk-copy (TMA engine) fed, warp-specialised, persistent with a dynamic tile counter (seg_gemm_tma.cu).
+// Needs every GEMM operand 16-byte aligned with an even leading dimension; `counter` is one device int of scratch.
+void launch_seg_gemm_tma(const Task* tasks, const Seg* segs, const Tile* tiles, int ntiles, int* counter, cudaStream_t st);
 
 // ---- vector kernels (Davidson; HBM-bound) ---------------------------------------------------------------------------
 // out[j] = sum_i x[i] * Y[j*ldy + i], j < m  (deterministic two-stage reduction; out is a device array of m doubles)
@@ -57,6 +61,10 @@ void launch_scale(double a, double* x, int64_t n, cudaStream_t st);
 struct DiagItemK { const double* ml; int ldl; const double* mr; int ldr; double c; };
 void launch_heff_diag(double* d, int nblocks, const int64_t* blk_off, const int* blk_rows, const int* blk_cols,
                       const int* item_ptr, const DiagItemK* items, cudaStream_t st);
+
+// dst block b (at dst_off[b], row stride pad2(cols[b])) = src block b (at src_off[b], packed [rows x cols]); pads untouched
+void launch_pad_blocks(double* dst, const double* src, int nblocks, const int64_t* dst_off, const int64_t* src_off,
+                       const int* rows, const int* cols, cudaStream_t st);
 
 // ---- small dense helpers ---------------------------------------------------------------------------------------------
 // out[c*rows + r] = in[r*ld_in + c]   (out is [cols x rows] contiguous)

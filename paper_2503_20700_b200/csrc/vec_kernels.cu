@@ -98,6 +98,22 @@ __global__ void __launch_bounds__(256) heff_diag_kernel(double* __restrict__ d, 
     }
 }
 
+// one CTA per block (grid-strided): packed [rows x cols] -> row stride pad2(cols)
+__global__ void __launch_bounds__(256) pad_blocks_kernel(double* __restrict__ dst, const double* __restrict__ src, int nblocks,
+                                                         const int64_t* __restrict__ doff, const int64_t* __restrict__ soff,
+                                                         const int* __restrict__ rows, const int* __restrict__ cols) {
+    for (int b = blockIdx.x; b < nblocks; b += gridDim.x) {
+        const int R = rows[b], Cc = cols[b], ld = (Cc + 1) & ~1;
+        const int64_t total = (int64_t)R * Cc;
+        const double* s = src + soff[b];
+        double* d = dst + doff[b];
+        for (int64_t e = threadIdx.x; e < total; e += blockDim.x) {
+            const int i = (int)(e / Cc), j = (int)(e % Cc);
+            d[(size_t)i * ld + j] = s[e];
+        }
+    }
+}
+
 __global__ void transpose_kernel(const double* __restrict__ in, int rows, int cols, int ld, double* __restrict__ out) {
     __shared__ double tile[32][33];
     const int c0 = blockIdx.x * 32, r0 = blockIdx.y * 32;
@@ -191,6 +207,11 @@ void launch_heff_diag(double* d, int nblocks, const int64_t* off, const int* row
                       const DiagItemK* items, cudaStream_t st) {
     if (nblocks <= 0) return;
     heff_diag_kernel<<<nblocks < 2368 ? nblocks : 2368, 256, 0, st>>>(d, nblocks, off, rows, cols, ptr, items);
+}
+void launch_pad_blocks(double* dst, const double* src, int nblocks, const int64_t* dst_off, const int64_t* src_off,
+                       const int* rows, const int* cols, cudaStream_t st) {
+    if (nblocks <= 0) return;
+    pad_blocks_kernel<<<nblocks < 2368 ? nblocks : 2368, 256, 0, st>>>(dst, src, nblocks, dst_off, src_off, rows, cols);
 }
 void launch_transpose(const double* in, int rows, int cols, int ld, double* out, cudaStream_t st) {
     if (rows <= 0 || cols <= 0) return;
