@@ -153,6 +153,15 @@ int dmrg_grouped_gemm(int ntasks, const int64_t* c_ptr, const int32_t* ldc, cons
                       const int64_t* a_ptr, const int64_t* b_ptr, const int32_t* lda, const int32_t* ldb,
                       const int32_t* kk, const int32_t* seg_flags, const double* alpha, void* cuda_stream);
 
+/* FP64 ceiling probe for the roofline denominator (SURVEY.md 8(d) D2 asks for a DMMA and a DFMA
+ * issue-rate microbenchmark and the cuBLAS DGEMM figure measured on the same box).  kind 0: register-resident
+ * DMMA.8x8x4 loop; 1: register-resident DFMA loop; 2: the DMMA loop fed from shared memory with the GEMM kernel's
+ * fragment pattern; 3: cublasDgemm size^3.  iters: inner iterations (kinds 0-2) or DGEMM calls per timing (kind 3);
+ * ctas_per_sm: resident 4-warp CTAs per SM (kinds 0-2).  Best of `reps` launches timed with CUDA events on
+ * `cuda_stream`; *tflops and *ms are HOST outputs.  Not part of the product path. */
+int dmrg_fp64_probe(int kind, int iters, int ctas_per_sm, int size, int reps, double* tflops, double* ms,
+                    void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

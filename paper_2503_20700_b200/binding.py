@@ -56,7 +56,7 @@ class dmrg_sweep_result(C.Structure):
 EXPORTS = ["dmrg_default_options", "dmrg_create", "dmrg_destroy", "dmrg_last_error", "dmrg_mps_import",
            "dmrg_mps_export", "dmrg_prepare_bond", "dmrg_heff_layout", "dmrg_heff_apply", "dmrg_heff_diag",
            "dmrg_heff_stats", "dmrg_sweep", "dmrg_rdm12", "dmrg_rdm_stats", "dmrg_launch_count", "dmrg_device_bytes",
-           "dmrg_grouped_gemm"]
+           "dmrg_grouped_gemm", "dmrg_fp64_probe"]
 
 lib.dmrg_last_error.restype = C.c_char_p
 lib.dmrg_last_error.argtypes = [C.c_void_p]
@@ -227,3 +227,13 @@ def dmrg_grouped_gemm(tasks, segs, stream=None):
     if rc != 0:
         raise DmrgError(rc, "dmrg_grouped_gemm failed")
     return rc
+
+
+def dmrg_fp64_probe(kind, iters=20000, ctas_per_sm=3, size=8192, reps=3, stream=None):
+    """FP64 ceiling probe (kind 0 DMMA, 1 DFMA, 2 DMMA fed by LDS, 3 cuBLAS DGEMM size^3): dict(tflops, ms)."""
+    tf, ms = C.c_double(0.0), C.c_double(0.0)
+    rc = lib.dmrg_fp64_probe(int(kind), int(iters), int(ctas_per_sm), int(size), int(reps), C.byref(tf), C.byref(ms),
+                             C.c_void_p(stream or 0))
+    if rc != 0:
+        raise DmrgError(rc, "dmrg_fp64_probe failed")
+    return {"tflops": tf.value, "ms": ms.value}

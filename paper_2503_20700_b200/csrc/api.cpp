@@ -404,4 +404,13 @@ int dmrg_grouped_gemm(int ntasks, const int64_t* c_ptr, const int32_t* ldc, cons
     return DMRG_OK;
 }
 
+int dmrg_fp64_probe(int kind, int iters, int ctas_per_sm, int size, int reps, double* tflops, double* ms,
+                    void* cuda_stream) {
+    if (kind < 0 || kind > 3 || iters < 1 || reps < 1 || !tflops || !ms) return DMRG_EINVAL;
+    if (kind < 3 && (ctas_per_sm < 1 || ctas_per_sm > 16)) return DMRG_EINVAL;
+    if (kind == 3 && (size < 1 || size > 32768)) return DMRG_EINVAL;
+    const int rc = fp64_probe(kind, iters, ctas_per_sm, size, reps, tflops, ms, (cudaStream_t)cuda_stream);
+    return rc == 0 ? DMRG_OK : (rc == -3 ? DMRG_ENOMEM : DMRG_ECUDA);
+}
+
 }  // extern "C"

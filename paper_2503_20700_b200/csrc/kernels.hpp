@@ -84,4 +84,7 @@ SvdWork* svd_create(cudaStream_t st);
 void svd_destroy(SvdWork* w);
 void svd_rowmajor(SvdWork* w, double* A, int m, int n, double* U, double* S, double* Vt, cudaStream_t st);
 
+// ---- FP64 ceiling probes (probe.cu; measurement only) -----------------------------------------------------------------
+int fp64_probe(int kind, int iters, int ctas_per_sm, int size, int reps, double* tflops, double* ms, cudaStream_t st);
+
 }  // namespace dmrg
