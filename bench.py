@@ -45,6 +45,7 @@ def parse_args():
     ap.add_argument("--cpu-baseline", type=int, default=1)
     ap.add_argument("--sample-config", type=int, default=2, help="config of the oracle's bounded sample")
     ap.add_argument("--sample-D", type=int, default=96)
+    ap.add_argument("--probe", type=int, default=1, help="1: run the FP64 ceiling probes (DMMA, DFMA, LDS-fed DMMA, cuBLAS DGEMM)")
     return ap.parse_args()
 
 
@@ -350,6 +351,16 @@ def run_ours(args):
             "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 8 * nnz, "d2h_bytes_per_step": 8 * nnz,
                     "ms_per_step": e2e_s * 1e3},
             "gpu_launches": int(launches), "clocks": clocks, "roofline": roof}
+    if args.probe:
+        # the ceilings the roofline fraction should be read against, measured in the same process on the same box
+        pr = {}
+        for name, kind, kw in (("dmma_regs", 0, {}), ("dfma_regs", 1, {}), ("dmma_lds", 2, {}),
+                               ("cublas_dgemm_8192", 3, dict(iters=2, size=8192))):
+            r = P.dmrg_fp64_probe(kind, **kw)
+            pr[name] = {"tflops": r["tflops"], "ms": r["ms"]}
+        pr["note"] = "kinds 0-2: 3 CTAs x 4 warps per SM, 16 independent DMMA.8x8x4 (or 32 DFMA) per warp per iteration"
+        line["fp64_probe"] = pr
+        roof["frac_of_dmma_probe"] = achieved / pr["dmma_regs"]["tflops"]
     if args.extras:
         line["extras"] = time_small_extras(P, torch)
     if args.cpu_baseline and world == 1:

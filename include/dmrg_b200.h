@@ -153,6 +153,10 @@ int dmrg_grouped_gemm(int ntasks, const int64_t* c_ptr, const int32_t* ldc, cons
                       const int64_t* a_ptr, const int64_t* b_ptr, const int32_t* lda, const int32_t* ldb,
                       const int32_t* kk, const int32_t* seg_flags, const double* alpha, void* cuda_stream);
 
+/* Device time in milliseconds (CUDA events on the call's stream around the kernel launch only, descriptor upload
+ * excluded) of the most recent dmrg_grouped_gemm call in this process. */
+double dmrg_last_gemm_ms(void);
+
 /* FP64 ceiling probe for the roofline denominator (SURVEY.md 8(d) D2 asks for a DMMA and a DFMA
  * issue-rate microbenchmark and the cuBLAS DGEMM figure measured on the same box).  kind 0: register-resident
  * DMMA.8x8x4 loop; 1: register-resident DFMA loop; 2: the DMMA loop fed from shared memory with the GEMM kernel's

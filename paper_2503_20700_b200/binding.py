@@ -56,12 +56,14 @@ class dmrg_sweep_result(C.Structure):
 EXPORTS = ["dmrg_default_options", "dmrg_create", "dmrg_destroy", "dmrg_last_error", "dmrg_mps_import",
            "dmrg_mps_export", "dmrg_prepare_bond", "dmrg_heff_layout", "dmrg_heff_apply", "dmrg_heff_diag",
            "dmrg_heff_stats", "dmrg_sweep", "dmrg_rdm12", "dmrg_rdm_stats", "dmrg_launch_count", "dmrg_device_bytes",
-           "dmrg_grouped_gemm", "dmrg_fp64_probe"]
+           "dmrg_grouped_gemm", "dmrg_last_gemm_ms", "dmrg_fp64_probe"]
 
 lib.dmrg_last_error.restype = C.c_char_p
 lib.dmrg_last_error.argtypes = [C.c_void_p]
 lib.dmrg_launch_count.restype = C.c_int64
 lib.dmrg_launch_count.argtypes = [C.c_void_p]
+lib.dmrg_last_gemm_ms.restype = C.c_double
+lib.dmrg_last_gemm_ms.argtypes = []
 lib.dmrg_device_bytes.restype = C.c_int64
 lib.dmrg_device_bytes.argtypes = [C.c_void_p]
 
@@ -237,3 +239,8 @@ def dmrg_fp64_probe(kind, iters=20000, ctas_per_sm=3, size=8192, reps=3, stream=
     if rc != 0:
         raise DmrgError(rc, "dmrg_fp64_probe failed")
     return {"tflops": tf.value, "ms": ms.value}
+
+
+def dmrg_last_gemm_ms():
+    """Device milliseconds of the kernel launched by the most recent dmrg_grouped_gemm call."""
+    return float(lib.dmrg_last_gemm_ms())

@@ -381,6 +381,9 @@ int dmrg_rdm_stats(dmrg_ctx* ctx, double* seconds, double* bytes_streamed, doubl
     API_END
 }
 
+static double g_last_gemm_ms = 0.0;
+double dmrg_last_gemm_ms(void) { return g_last_gemm_ms; }
+
 int dmrg_grouped_gemm(int ntasks, const int64_t* c_ptr, const int32_t* ldc, const int32_t* m, const int32_t* n,
                       const int32_t* seg_begin, const int32_t* seg_count, const int32_t* task_flags, int nsegs,
                       const int64_t* a_ptr, const int64_t* b_ptr, const int32_t* lda, const int32_t* ldb,
@@ -398,7 +401,22 @@ int dmrg_grouped_gemm(int ntasks, const int64_t* c_ptr, const int32_t* ldc, cons
                 b.add_seg(t, (const double*)(uintptr_t)a_ptr[s], lda[s], (const double*)(uintptr_t)b_ptr[s], ldb[s], kk[s],
                           seg_flags[s], alpha[s]);
         }
-        run_once(b, tmp);
+        if (!b.tasks.empty()) {
+            GemmLaunch l;
+            finalize(b, l, tmp);
+            cudaEvent_t e0, e1;
+            cuda_check(cudaEventCreate(&e0), "event");
+            cuda_check(cudaEventCreate(&e1), "event");
+            cudaEventRecord(e0, tmp.stream);
+            run(l, tmp);
+            cudaEventRecord(e1, tmp.stream);
+            cuda_check(cudaStreamSynchronize(tmp.stream), "grouped GEMM");
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, e0, e1);
+            g_last_gemm_ms = ms;
+            cudaEventDestroy(e0);
+            cudaEventDestroy(e1);
+        }
     } catch (const Error& e) { return e.code; }
     catch (...) { return DMRG_ECUDA; }
     return DMRG_OK;

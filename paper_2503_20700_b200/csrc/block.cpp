@@ -71,6 +71,7 @@ int GemmBatch::add_task(double* C, int ldc, int M, int N, int flags) {
 }
 void GemmBatch::add_seg(int task, const double* A, int lda, const double* B, int ldb, int K, int flags,
                         double alpha) {
+    if (!(flags & SEG_IDENT_B) && K <= 0) return;            // an empty product contributes nothing (kernels assume K >= 1)
     Seg s;
     s.A = A; s.B = B; s.lda = lda; s.ldb = ldb; s.K = K; s.flags = flags; s.alpha = alpha;
     segs.push_back(s);
@@ -120,9 +121,13 @@ void finalize(GemmBatch& b, GemmLaunch& out, Engine& eng) {
     for (int t : order) {
         const Task& tk = b.tasks[t];
         if (tk.M <= 0 || tk.N <= 0) continue;
+        // even split of each extent into ceil(extent / 64) pieces rounded up to the 8-row DMMA fragment: the kernel
+        // skips fragments outside [mv x nv], so the padding waste is at the 8 level, not the 64 level
         const int nm = (tk.M + GEMM_BM - 1) / GEMM_BM, nn = (tk.N + GEMM_BN - 1) / GEMM_BN;
-        for (int i = 0; i < nm; ++i)
-            for (int j = 0; j < nn; ++j) tiles.push_back({t, i, j});
+        const int pm = std::min(GEMM_BM, (((tk.M + nm - 1) / nm) + 7) & ~7), pn = std::min(GEMM_BN, (((tk.N + nn - 1) / nn) + 7) & ~7);
+        for (int m0 = 0; m0 < tk.M; m0 += pm)
+            for (int n0 = 0; n0 < tk.N; n0 += pn)
+                tiles.push_back({t, m0, n0, std::min(pm, tk.M - m0), std::min(pn, tk.N - n0)});
     }
     out.tasks.upload(b.tasks, eng.stream);
     out.segs.upload(sorted, eng.stream);

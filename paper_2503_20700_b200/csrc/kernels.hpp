@@ -34,8 +34,8 @@ struct Task {
     int flags;
     int ngemm;                  // segments [seg_begin, seg_begin + ngemm) are GEMM segments, the rest identity-B (set by finalize)
 };
-struct Tile {
-    int task, tm, tn;
+struct Tile {                   // output tile [m0, m0+mv) x [n0, n0+nv) of a task; m0, n0 multiples of 8, mv <= BM, nv <= BN
+    int task, m0, n0, mv, nv;
 };
 constexpr int GEMM_BM = 64, GEMM_BN = 64, GEMM_BK = 16, GEMM_THREADS = 128, GEMM_STAGES = 4;
 

@@ -92,8 +92,7 @@ __global__ void __launch_bounds__(NT) seg_gemm_kernel(const Task* __restrict__ t
         const Task tk = tasks[tl.task];
         const Seg* sg = segs + tk.seg_begin;
         const int nseg = tk.seg_count;
-        const int m0 = tl.tm * BM, n0 = tl.tn * BN;
-        const int mv = min(BM, tk.M - m0), nv = min(BN, tk.N - n0);
+        const int m0 = tl.m0, n0 = tl.n0, mv = tl.mv, nv = tl.nv;
 
         double acc[4][4][2], tmp[4][4][2];
 #pragma unroll
@@ -204,13 +203,13 @@ __global__ void __launch_bounds__(NT) seg_gemm_kernel(const Task* __restrict__ t
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             const int row = m0 + wm + 8 * i + fr;
-            if (row >= tk.M) continue;
+            if (row >= m0 + mv) continue;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 const int col = n0 + wn + 8 * j + 2 * fc;
-                if (col >= tk.N) continue;
+                if (col >= n0 + nv) continue;
                 double v0 = acc[i][j][0], v1 = acc[i][j][1];
-                const bool two = (col + 1 < tk.N);
+                const bool two = (col + 1 < n0 + nv);
                 for (int s = 0; s < nseg; ++s) {
                     if (!(sg[s].flags & SEG_IDENT_B)) continue;
                     const double* ap = sg[s].A + (size_t)row * sg[s].lda + col;

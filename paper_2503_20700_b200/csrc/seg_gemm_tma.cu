@@ -36,11 +36,16 @@ enum : int { F_TA = 1, F_TB = 2, F_FIRST = 4, F_LAST = 8, F_COMPUTE = 16, F_STOP
 struct StageInfo {                             // written by the producer, read by the consumers
     double alpha;
     int flags, kv;
-    // tile fields, valid when F_FIRST is set
+    int tslot, pad;                            // slot of the tile in the tile ring, valid when F_FIRST is set
+};
+// Tile parameters live in a shared ring instead of consumer registers.  A tile occupies at least one stage and the
+// producer runs at most ST2 stages ahead of the slowest consumer, so ST2 + 1 slots can never be overwritten early.
+struct TileInfo {
     double* C;
     const Seg* ident;                          // identity-B segments of the task
-    int ldc, M, N, m0, n0, tflags, nident, pad;
+    int ldc, mv, nv, m0, n0, tflags, nident, pad;   // output tile [m0, m0+mv) x [n0, n0+nv)
 };
+constexpr int NTR = ST2 + 1;
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -86,12 +91,43 @@ __device__ __forceinline__ void dmma(double& d0, double& d1, double a, double b)
 __device__ __forceinline__ int pad2d(int n) { return (n + 1) & ~1; }
 
 
+// One full-K pipeline stage for a warp that owns NI x NJ fragments: fully unrolled, no predicates.  Every ragged tile
+// shape gets its own straight-line DMMA sequence, so skipping fragments costs nothing in the instruction stream.
+template <int NI, int NJ>
+__device__ __forceinline__ void mma_stage(double (&acc)[4][4][2], const double* __restrict__ As,
+                                          const double* __restrict__ Bs, int a_off, int a_ks, int a_ms, int b_off,
+                                          int b_ks, int b_ns, double al) {
+#pragma unroll
+    for (int kk = 0; kk < BK; kk += 4) {
+        double a[NI], b[NJ];
+#pragma unroll
+        for (int i = 0; i < NI; ++i) a[i] = al * As[a_off + kk * a_ks + 8 * i * a_ms];
+#pragma unroll
+        for (int j = 0; j < NJ; ++j) b[j] = Bs[b_off + kk * b_ks + 8 * j * b_ns];
+#pragma unroll
+        for (int i = 0; i < NI; ++i)
+#pragma unroll
+            for (int j = 0; j < NJ; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+    }
+}
+template <int NI>
+__device__ __forceinline__ void mma_stage_nj(int nj, double (&acc)[4][4][2], const double* As, const double* Bs,
+                                             int a_off, int a_ks, int a_ms, int b_off, int b_ks, int b_ns, double al) {
+    switch (nj) {
+        case 4: mma_stage<NI, 4>(acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, al); break;
+        case 3: mma_stage<NI, 3>(acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, al); break;
+        case 2: mma_stage<NI, 2>(acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, al); break;
+        default: mma_stage<NI, 1>(acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, al); break;
+    }
+}
+
 __global__ void __launch_bounds__(NT2, 3)
 seg_gemm_tma_kernel(const Task* __restrict__ tasks, const Seg* __restrict__ segs, const Tile* __restrict__ tiles,
                     int ntiles, int* __restrict__ counter) {
     extern __shared__ __align__(128) double smem[];
     __shared__ __align__(8) uint64_t full_bar[ST2], empty_bar[ST2];
     __shared__ StageInfo info[ST2];
+    __shared__ TileInfo tring[NTR];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) {
@@ -102,40 +138,56 @@ seg_gemm_tma_kernel(const Task* __restrict__ tasks, const Seg* __restrict__ segs
 
     if (warp == NCONS) {
         // ===================================== producer warp ==========================================================
+        // Descriptor pipeline: the dependent chain  tile counter -> Tile -> Task -> first Seg  is spread over four
+        // tiles (each load is issued one tile before its result is needed), and inside a tile the next Seg is loaded
+        // while the current one is being streamed, so the producer never waits on descriptor latency in steady state.
         uint32_t pstep = 0;
-        for (;;) {
-            int tile_id = 0;
-            if (lane == 0) tile_id = atomicAdd(counter, 1);
-            tile_id = __shfl_sync(0xffffffffu, tile_id, 0);
-            const bool stop = tile_id >= ntiles;
-            Tile tl;
-            Task tk;
+        int tslot = 0;
+        auto take = [&]() { int v = 0; if (lane == 0) v = atomicAdd(counter, 1); return v; };   // valid on lane 0
+        Tile tl_d, tl_c, tl_b;
+        Task tk_d, tk_c;
+        Seg sg_d;
+        int id_d, id_c, id_b, id_a;
+        id_d = __shfl_sync(0xffffffffu, take(), 0);
+        id_c = __shfl_sync(0xffffffffu, take(), 0);
+        id_b = __shfl_sync(0xffffffffu, take(), 0);
+        id_a = take();
+        if (id_d < ntiles) { tl_d = tiles[id_d]; tk_d = tasks[tl_d.task]; if (tk_d.ngemm > 0) sg_d = segs[tk_d.seg_begin]; }
+        if (id_c < ntiles) { tl_c = tiles[id_c]; tk_c = tasks[tl_c.task]; }
+        if (id_b < ntiles) tl_b = tiles[id_b];
+        for (;; tslot = (tslot + 1 == NTR) ? 0 : tslot + 1) {
+            const bool stop = id_d >= ntiles;
+            const Tile tl = tl_d;
+            const Task tk = tk_d;
+            Seg cur = sg_d, nxt;
+            // advance the pipeline (every use below is of a load issued one tile ago)
+            id_d = id_c; tl_d = tl_c; tk_d = tk_c;
+            if (id_d < ntiles && tk_d.ngemm > 0) sg_d = segs[tk_d.seg_begin];
+            id_c = id_b; tl_c = tl_b;
+            if (id_c < ntiles) tk_c = tasks[tl_c.task];
+            id_b = __shfl_sync(0xffffffffu, id_a, 0);
+            if (id_b < ntiles) tl_b = tiles[id_b];
+            if (!stop) id_a = take();
             const Seg* sg = nullptr;
             int m0 = 0, n0 = 0, mv = 0, nv = 0, lastseg = -1;
             if (!stop) {
-                tl = tiles[tile_id];
-                tk = tasks[tl.task];
                 sg = segs + tk.seg_begin;
-                m0 = tl.tm * BM; n0 = tl.tn * BN;
-                mv = min(BM, tk.M - m0); nv = min(BN, tk.N - n0);
-                lastseg = tk.ngemm - 1;
-                while (lastseg >= 0 && sg[lastseg].K <= 0) --lastseg;
+                m0 = tl.m0; n0 = tl.n0; mv = tl.mv; nv = tl.nv;
+                lastseg = tk.ngemm - 1;                       // the host drops empty (K <= 0) GEMM segments
             }
             bool first = true;
             int s = 0, lk = 0;
-            while (!stop && s <= lastseg && sg[s].K <= 0) ++s;
+            if (lastseg >= 1) nxt = sg[1];
             do {                                              // one pipeline stage per iteration
                 const int stage = pstep % ST2;
                 mbar_wait(&empty_bar[stage], ((pstep / ST2) & 1) ^ 1);
                 double* As = smem + stage * STAGE_DOUBLES;
                 double* Bs = As + PANEL;
                 const bool compute = !stop && s <= lastseg;
-                Seg cur;
                 int kv = 0, rowsA = 0, rowsB = 0;
                 uint32_t bytesA = 0, bytesB = 0;
                 bool last = true;
                 if (compute) {
-                    cur = sg[s];
                     kv = min(BK, cur.K - lk);
                     if (cur.flags & SEG_TRANS_A) { rowsA = kv; bytesA = (uint32_t)pad2d(mv) * 8u; }    // bulk rows [k][m]
                     if (!(cur.flags & SEG_TRANS_B)) { rowsB = kv; bytesB = (uint32_t)pad2d(nv) * 8u; } // bulk rows [k][n]
@@ -148,8 +200,10 @@ seg_gemm_tma_kernel(const Task* __restrict__ tasks, const Seg* __restrict__ segs
                     in.flags = stop ? F_STOP
                                     : ((compute ? (F_COMPUTE | (cur.flags & 3)) : 0) | (first ? F_FIRST : 0) | (last ? F_LAST : 0));
                     if (first && !stop) {
-                        in.C = tk.C; in.ident = sg + tk.ngemm; in.nident = tk.seg_count - tk.ngemm;
-                        in.ldc = tk.ldc; in.M = tk.M; in.N = tk.N; in.m0 = m0; in.n0 = n0; in.tflags = tk.flags;
+                        TileInfo& ti = tring[tslot];
+                        ti.C = tk.C; ti.ident = sg + tk.ngemm; ti.nident = tk.seg_count - tk.ngemm;
+                        ti.ldc = tk.ldc; ti.mv = mv; ti.nv = nv; ti.m0 = m0; ti.n0 = n0; ti.tflags = tk.flags;
+                        in.tslot = tslot;
                     }
                     mbar_arrive_expect_tx(&full_bar[stage], (uint32_t)rowsA * bytesA + (uint32_t)rowsB * bytesB);
                 }
@@ -179,10 +233,11 @@ seg_gemm_tma_kernel(const Task* __restrict__ tasks, const Seg* __restrict__ segs
                         for (int r = lane; r < rowsB; r += 32) bulk_g2s(Bs + r * LDM, src + (size_t)r * cur.ldb, bytesB, &full_bar[stage]);
                     }
                     lk += BK;
-                    if (lk >= cur.K) {
+                    if (lk >= cur.K) {                                // next segment: already in registers
                         lk = 0;
                         ++s;
-                        while (s <= lastseg && sg[s].K <= 0) ++s;
+                        cur = nxt;
+                        if (s + 1 <= lastseg) nxt = sg[s + 1];
                     }
                 }
                 ldgsts_arrive_noinc(&full_bar[stage]);                // fires when this lane's LDGSTS of the stage have landed
@@ -195,13 +250,13 @@ seg_gemm_tma_kernel(const Task* __restrict__ tasks, const Seg* __restrict__ segs
     }
 
     // ========================================= consumer warps ==========================================================
-    const int wm = (warp >> 1) * 32, wn = (warp & 1) * 32;
+    // The tile's ceil(mv/8) x ceil(nv/8) DMMA fragments are split evenly over the 2 x 2 warps (each at most 4 x 4);
+    // fragments outside the tile are never issued, so ragged sector dimensions waste at most 7 rows / columns.
     const int fr = lane >> 2, fc = lane & 3;              // fragment row (0..7) and k / column-pair index (0..3)
     double acc[4][4][2];
-    double* tC = nullptr;
-    const Seg* tident = nullptr;
-    int tldc = 0, tM = 0, tN = 0, tm0 = 0, tn0 = 0, tflags = 0, tnident = 0;
-    uint32_t cstep = 0;
+    int cslot = 0;                                        // tile ring slot of the current tile
+    int wm = 0, wn = 0, ni = 0, nj = 0;                   // this warp's fragment origin and counts within the tile
+    uint32_t cstep = 0, rot = blockIdx.x;
     for (;; ++cstep) {
         const int stage = cstep % ST2;
         mbar_wait(&full_bar[stage], (cstep / ST2) & 1);
@@ -209,8 +264,14 @@ seg_gemm_tma_kernel(const Task* __restrict__ tasks, const Seg* __restrict__ segs
         const int fl = in.flags;
         if (fl & F_STOP) break;
         if (fl & F_FIRST) {
-            tC = in.C; tident = in.ident; tnident = in.nident;
-            tldc = in.ldc; tM = in.M; tN = in.N; tm0 = in.m0; tn0 = in.n0; tflags = in.tflags;
+            cslot = in.tslot;
+            const int tmv = tring[cslot].mv, tnv = tring[cslot].nv;
+            const int fm = (tmv + 7) >> 3, fn = (tnv + 7) >> 3, hm = (fm + 1) >> 1, hn = (fn + 1) >> 1;
+            // the quadrant a warp takes rotates from tile to tile: the heavier quadrants of ragged tiles visit every
+            // warp (and with it every SM sub-partition's DMMA pipe) equally often
+            const int role = (warp + (int)(rot++)) & 3;
+            wm = (role >> 1) ? hm * 8 : 0; ni = (role >> 1) ? fm - hm : hm;
+            wn = (role & 1) ? hn * 8 : 0;  nj = (role & 1) ? fn - hn : hn;
 #pragma unroll
             for (int i = 0; i < 4; ++i)
 #pragma unroll
@@ -227,31 +288,33 @@ seg_gemm_tma_kernel(const Task* __restrict__ tasks, const Seg* __restrict__ segs
             const int b_off = (fl & F_TB) ? ((wn + fr) * LDK + fc) : (fc * LDM + wn + fr);
             const int b_ks = (fl & F_TB) ? 1 : LDM;
             const int b_ns = (fl & F_TB) ? LDK : 1;
-            if (kv == BK) {
+            if (ni == 0 || nj == 0) {
+                // nothing to do for this warp in this tile
+            } else if (kv == BK) {
+                switch (ni) {
+                    case 4: mma_stage_nj<4>(nj, acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, al); break;
+                    case 3: mma_stage_nj<3>(nj, acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, al); break;
+                    case 2: mma_stage_nj<2>(nj, acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, al); break;
+                    default: mma_stage_nj<1>(nj, acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, al); break;
+                }
+            } else {                                         // ragged K tail (masked in registers; once per segment)
 #pragma unroll
                 for (int kk = 0; kk < BK; kk += 4) {
-                    double a[4], b[4];
+                    if (kk < kv) {
+                        const bool ok = kk + fc < kv;
+                        double a[4], b[4];
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) a[i] = al * As[a_off + kk * a_ks + 8 * i * a_ms];
+                        for (int i = 0; i < 4; ++i) { const double v = As[a_off + kk * a_ks + 8 * i * a_ms]; a[i] = ok ? al * v : 0.0; }
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) b[j] = Bs[b_off + kk * b_ks + 8 * j * b_ns];
+                        for (int j = 0; j < 4; ++j) { const double v = Bs[b_off + kk * b_ks + 8 * j * b_ns]; b[j] = ok ? v : 0.0; }
 #pragma unroll
-                    for (int i = 0; i < 4; ++i)
+                        for (int i = 0; i < 4; ++i)
+                            if (i < ni) {
 #pragma unroll
-                        for (int j = 0; j < 4; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
-                }
-            } else {                                         // ragged K tail: mask both fragments in registers
-                for (int kk = 0; kk < kv; kk += 4) {
-                    const bool ok = kk + fc < kv;
-                    double a[4], b[4];
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) { const double v = As[a_off + kk * a_ks + 8 * i * a_ms]; a[i] = ok ? al * v : 0.0; }
-#pragma unroll
-                    for (int j = 0; j < 4; ++j) { const double v = Bs[b_off + kk * b_ks + 8 * j * b_ns]; b[j] = ok ? v : 0.0; }
-#pragma unroll
-                    for (int i = 0; i < 4; ++i)
-#pragma unroll
-                        for (int j = 0; j < 4; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+                                for (int j = 0; j < 4; ++j)
+                                    if (j < nj) dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+                            }
+                    }
                 }
             }
         }
@@ -259,18 +322,22 @@ seg_gemm_tma_kernel(const Task* __restrict__ tasks, const Seg* __restrict__ segs
         if (lane == 0) mbar_arrive(&empty_bar[stage]);       // this warp is done with the stage (data and info)
         if (fl & F_LAST) {
             // ---- epilogue: identity-B segments, optional accumulate, store ------------------------------------------
-            const bool accum = tflags & TASK_ACCUM;
+            const TileInfo& ti = tring[cslot];
+            double* const tC = ti.C;
+            const Seg* const tident = ti.ident;
+            const int tldc = ti.ldc, tnident = ti.nident, tm0 = ti.m0, tn0 = ti.n0, tmv = ti.mv, tnv = ti.nv;
+            const bool accum = ti.tflags & TASK_ACCUM;
             const bool al_c = ((((uintptr_t)tC) & 15) == 0) && ((tldc & 1) == 0);
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
                 const int row = tm0 + wm + 8 * i + fr;
-                if (row >= tM) continue;
+                if (i >= ni || row >= tm0 + tmv) continue;
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
                     const int col = tn0 + wn + 8 * j + 2 * fc;
-                    if (col >= tN) continue;
+                    if (j >= nj || col >= tn0 + tnv) continue;
                     double v0 = acc[i][j][0], v1 = acc[i][j][1];
-                    const bool two = (col + 1 < tN);
+                    const bool two = (col + 1 < tn0 + tnv);
                     for (int s = 0; s < tnident; ++s) {
                         const double* ap = tident[s].A + (size_t)row * tident[s].lda + col;
                         v0 += tident[s].alpha * ap[0];
