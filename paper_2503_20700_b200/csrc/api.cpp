@@ -111,6 +111,7 @@ int dmrg_create(dmrg_ctx** out, int k, int n_elec, int two_sz, const double* h, 
         eng.ham.eri.assign(eri, eri + (size_t)k * k * k * k);
         eng.svd = svd_create(eng.stream);
         { const char* g = std::getenv("DMRG_B200_GENERIC_GEMM"); eng.force_generic_gemm = g && g[0] == '1'; }
+        { const char* g = std::getenv("DMRG_B200_TRACE"); eng.trace = g && g[0] == '1'; }
     } catch (...) {
         delete ctx;
         return DMRG_ECUDA;

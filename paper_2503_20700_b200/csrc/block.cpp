@@ -71,7 +71,6 @@ int GemmBatch::add_task(double* C, int ldc, int M, int N, int flags) {
 }
 void GemmBatch::add_seg(int task, const double* A, int lda, const double* B, int ldb, int K, int flags,
                         double alpha) {
-    if (!(flags & SEG_IDENT_B) && K <= 0) return;            // an empty product contributes nothing (kernels assume K >= 1)
     Seg s;
     s.A = A; s.B = B; s.lda = lda; s.ldb = ldb; s.K = K; s.flags = flags; s.alpha = alpha;
     segs.push_back(s);
@@ -81,20 +80,33 @@ void GemmBatch::add_seg(int task, const double* A, int lda, const double* B, int
 
 void finalize(GemmBatch& b, GemmLaunch& out, Engine& eng) {
     const int nt = (int)b.tasks.size();
-    for (auto& t : b.tasks) t.seg_count = 0;
-    for (int t : b.seg_task) b.tasks[t].seg_count++;
-    int run = 0;
-    for (auto& t : b.tasks) { t.seg_begin = run; run += t.seg_count; }
-    std::vector<Seg> sorted(b.segs.size());
-    std::vector<int> cursor(nt);
-    for (int t = 0; t < nt; ++t) cursor[t] = b.tasks[t].seg_begin;
-    // stable within a task, GEMM segments first, identity-B segments last
-    for (auto& t : b.tasks) t.ngemm = 0;
-    for (size_t j = 0; j < b.segs.size(); ++j)
-        if (!(b.segs[j].flags & SEG_IDENT_B)) sorted[cursor[b.seg_task[j]]++] = b.segs[j];
-    for (int t = 0; t < nt; ++t) b.tasks[t].ngemm = cursor[t] - b.tasks[t].seg_begin;
-    for (size_t j = 0; j < b.segs.size(); ++j)
-        if (b.segs[j].flags & SEG_IDENT_B) sorted[cursor[b.seg_task[j]]++] = b.segs[j];
+    // Order within a task: GEMM segments first, sorted by alpha (stable), identity-B segments last.  Empty products
+    // (K <= 0 or alpha == 0) are dropped.  Equal alphas adjacent let the bulk-copy kernel keep its accumulators in
+    // units of the current alpha and rescale them only when alpha changes (no per-fragment multiply in the main loop).
+    std::vector<std::vector<int>> by_task(nt);
+    for (size_t j = 0; j < b.segs.size(); ++j) {
+        const Seg& sg = b.segs[j];
+        if (!(sg.flags & SEG_IDENT_B) && (sg.K <= 0 || sg.alpha == 0.0)) continue;
+        by_task[b.seg_task[j]].push_back((int)j);
+    }
+    std::vector<Seg> sorted;
+    sorted.reserve(b.segs.size());
+    for (int t = 0; t < nt; ++t) {
+        std::vector<int>& v = by_task[t];
+        std::stable_sort(v.begin(), v.end(), [&](int x, int y) {
+            const bool ix = b.segs[x].flags & SEG_IDENT_B, iy = b.segs[y].flags & SEG_IDENT_B;
+            if (ix != iy) return iy;
+            if (ix) return false;
+            return b.segs[x].alpha < b.segs[y].alpha;
+        });
+        b.tasks[t].seg_begin = (int)sorted.size();
+        b.tasks[t].seg_count = (int)v.size();
+        b.tasks[t].ngemm = 0;
+        for (int j : v) {
+            if (!(b.segs[j].flags & SEG_IDENT_B)) b.tasks[t].ngemm++;
+            sorted.push_back(b.segs[j]);
+        }
+    }
     bool aligned = true;
     for (const Seg& sg : sorted) {
         if (sg.flags & SEG_IDENT_B) continue;
@@ -114,11 +126,11 @@ void finalize(GemmBatch& b, GemmLaunch& out, Engine& eng) {
     std::vector<double> weight(nt, 0.0);
     for (int t = 0; t < nt; ++t)
         for (int j = 0; j < b.tasks[t].seg_count; ++j) weight[t] += sorted[b.tasks[t].seg_begin + j].K;
-    std::vector<int> order(nt);
-    for (int t = 0; t < nt; ++t) order[t] = t;
-    std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return weight[x] > weight[y]; });
-    std::vector<Tile> tiles;
-    for (int t : order) {
+    // tiles, heaviest first (weight = K extent x DMMA fragments of the tile) so that the persistent kernel's dynamic
+    // tile counter ends the launch on short tiles
+    std::vector<Tile> raw;
+    std::vector<double> tw;
+    for (int t = 0; t < nt; ++t) {
         const Task& tk = b.tasks[t];
         if (tk.M <= 0 || tk.N <= 0) continue;
         // even split of each extent into ceil(extent / 64) pieces rounded up to the 8-row DMMA fragment: the kernel
@@ -126,9 +138,17 @@ void finalize(GemmBatch& b, GemmLaunch& out, Engine& eng) {
         const int nm = (tk.M + GEMM_BM - 1) / GEMM_BM, nn = (tk.N + GEMM_BN - 1) / GEMM_BN;
         const int pm = std::min(GEMM_BM, (((tk.M + nm - 1) / nm) + 7) & ~7), pn = std::min(GEMM_BN, (((tk.N + nn - 1) / nn) + 7) & ~7);
         for (int m0 = 0; m0 < tk.M; m0 += pm)
-            for (int n0 = 0; n0 < tk.N; n0 += pn)
-                tiles.push_back({t, m0, n0, std::min(pm, tk.M - m0), std::min(pn, tk.N - n0)});
+            for (int n0 = 0; n0 < tk.N; n0 += pn) {
+                const int mv = std::min(pm, tk.M - m0), nv = std::min(pn, tk.N - n0);
+                raw.push_back({t, m0, n0, mv, nv});
+                tw.push_back((weight[t] + 16.0) * ((mv + 7) / 8) * ((nv + 7) / 8));
+            }
     }
+    std::vector<int> order(raw.size());
+    for (size_t j = 0; j < raw.size(); ++j) order[j] = (int)j;
+    std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return tw[x] > tw[y]; });
+    std::vector<Tile> tiles(raw.size());
+    for (size_t j = 0; j < raw.size(); ++j) tiles[j] = raw[order[j]];
     out.tasks.upload(b.tasks, eng.stream);
     out.segs.upload(sorted, eng.stream);
     out.tiles.upload(tiles, eng.stream);
@@ -139,11 +159,25 @@ void finalize(GemmBatch& b, GemmLaunch& out, Engine& eng) {
 }
 void run(const GemmLaunch& l, Engine& eng) {
     if (l.ntiles == 0) return;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (eng.trace) {                                           // DMRG_B200_TRACE=1: per-launch device time on stderr
+        cudaEventCreate(&e0); cudaEventCreate(&e1);
+        cudaEventRecord(e0, eng.stream);
+    }
     if (l.aligned && !eng.force_generic_gemm)
         launch_seg_gemm_tma(l.tasks.p, l.segs.p, l.tiles.p, l.ntiles, l.counter.p, eng.stream);
     else
         launch_seg_gemm(l.tasks.p, l.segs.p, l.tiles.p, l.ntiles, eng.stream);
     eng.launches++;
+    if (eng.trace) {
+        cudaEventRecord(e1, eng.stream);
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        std::fprintf(stderr, "[dmrg trace] gemm %s tiles=%d tasks=%zu segs=%zu flops=%.4e ms=%.3f tflops=%.2f\n",
+                     l.aligned ? "tma" : "generic", l.ntiles, l.tasks.n, l.segs.n, l.flops, ms, l.flops / (ms * 1e-3) / 1e12);
+        cudaEventDestroy(e0); cudaEventDestroy(e1);
+    }
 }
 void run_once(GemmBatch& b, Engine& eng) {
     if (b.tasks.empty()) return;

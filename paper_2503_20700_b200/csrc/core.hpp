@@ -215,6 +215,7 @@ struct Engine {
     double rdm_seconds = 0, rdm_bytes = 0, rdm_flops = 0;
     bool keep_env_stack = true;
     bool sweep_ready = false;                     // environments consistent with the sweep position
+    bool trace = false;                           // DMRG_B200_TRACE=1: print every grouped-GEMM launch's device time
     bool force_generic_gemm = false;              // DMRG_B200_GENERIC_GEMM=1: always the cp.async kernel (A/B testing)
     char mode_L(int b) const { return b <= bsw ? 'N' : 'C'; }
     char mode_R(int b) const { return b >= bsw + 3 ? 'N' : 'C'; }

@@ -22,19 +22,32 @@ namespace dmrg {
 
 namespace {
 
-constexpr int BM = GEMM_BM, BN = GEMM_BN, BK = GEMM_BK;
+#ifndef TMA_BK
+#define TMA_BK 16
+#endif
+#ifndef TMA_ST
+#define TMA_ST 3
+#endif
+#ifndef TMA_CPS
+#define TMA_CPS 3
+#endif
+constexpr int BM = GEMM_BM, BK = TMA_BK;      // CTA tile 64 x 64, K step of one pipeline stage
 constexpr int NCONS = 4;                       // consumer warps
 constexpr int NT2 = (NCONS + 1) * 32;          // + one producer warp
-constexpr int ST2 = 3;                         // pipeline stages (60 KB per CTA: three CTAs per SM)
+constexpr int ST2 = TMA_ST;                    // pipeline stages (BK 16: 20 KB each, 60 KB per CTA, three CTAs per SM)
+constexpr int CPS = TMA_CPS;                   // resident CTAs per SM the register budget is cut for
 constexpr int LDK = BK + 4;                    // row stride of the [m][k] / [n][k] layouts (160 B)
 constexpr int LDM = BM + 4;                    // row stride of the [k][m] / [k][n] layouts (544 B)
-constexpr int PANEL = BM * LDK;                // 1280 doubles >= BK * LDM = 1088
+constexpr int PANEL = (BM * LDK > BK * LDM) ? BM * LDK : BK * LDM;
+constexpr int LCPR = BK / 2;                   // LDGSTS: 16-byte chunks per [m][k] panel row = lanes per row
+constexpr int LRS = 32 / LCPR;                 // LDGSTS: panel rows covered by one warp instruction
 constexpr int STAGE_DOUBLES = 2 * PANEL;
 
-enum : int { F_TA = 1, F_TB = 2, F_FIRST = 4, F_LAST = 8, F_COMPUTE = 16, F_STOP = 32 };
+enum : int { F_TA = 1, F_TB = 2, F_FIRST = 4, F_LAST = 8, F_COMPUTE = 16, F_STOP = 32, F_RESCALE = 64 };
 
 struct StageInfo {                             // written by the producer, read by the consumers
-    double alpha;
+    double alpha;                              // alpha of the stage's segment: the accumulators are kept in units of it
+    double ratio;                              // F_RESCALE: previous alpha / alpha, applied to the accumulators first
     int flags, kv;
     int tslot, pad;                            // slot of the tile in the tile ring, valid when F_FIRST is set
 };
@@ -91,37 +104,57 @@ __device__ __forceinline__ void dmma(double& d0, double& d1, double a, double b)
 __device__ __forceinline__ int pad2d(int n) { return (n + 1) & ~1; }
 
 
-// One full-K pipeline stage for a warp that owns NI x NJ fragments: fully unrolled, no predicates.  Every ragged tile
+// One pipeline stage for a warp that owns NI x NJ fragments: fully unrolled, no predicated DMMA.  Every ragged tile
 // shape gets its own straight-line DMMA sequence, so skipping fragments costs nothing in the instruction stream.
-template <int NI, int NJ>
+// FULL: all BK columns valid.  Otherwise the k-steps at or beyond kv are skipped (warp-uniform branch around whole
+// steps) and the last partial step is masked in registers.
+template <int NI, int NJ, bool FULL>
 __device__ __forceinline__ void mma_stage(double (&acc)[4][4][2], const double* __restrict__ As,
                                           const double* __restrict__ Bs, int a_off, int a_ks, int a_ms, int b_off,
-                                          int b_ks, int b_ns, double al) {
+                                          int b_ks, int b_ns, int kv, int fc) {
 #pragma unroll
     for (int kk = 0; kk < BK; kk += 4) {
+        if (!FULL && kk >= kv) break;
         double a[NI], b[NJ];
 #pragma unroll
-        for (int i = 0; i < NI; ++i) a[i] = al * As[a_off + kk * a_ks + 8 * i * a_ms];
+        for (int i = 0; i < NI; ++i) a[i] = As[a_off + kk * a_ks + 8 * i * a_ms];
 #pragma unroll
         for (int j = 0; j < NJ; ++j) b[j] = Bs[b_off + kk * b_ks + 8 * j * b_ns];
+        if (!FULL && kk + fc >= kv) {
+#pragma unroll
+            for (int i = 0; i < NI; ++i) a[i] = 0.0;
+#pragma unroll
+            for (int j = 0; j < NJ; ++j) b[j] = 0.0;
+        }
 #pragma unroll
         for (int i = 0; i < NI; ++i)
 #pragma unroll
             for (int j = 0; j < NJ; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
     }
 }
-template <int NI>
+template <int NI, bool FULL>
 __device__ __forceinline__ void mma_stage_nj(int nj, double (&acc)[4][4][2], const double* As, const double* Bs,
-                                             int a_off, int a_ks, int a_ms, int b_off, int b_ks, int b_ns, double al) {
+                                             int a_off, int a_ks, int a_ms, int b_off, int b_ks, int b_ns, int kv, int fc) {
     switch (nj) {
-        case 4: mma_stage<NI, 4>(acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, al); break;
-        case 3: mma_stage<NI, 3>(acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, al); break;
-        case 2: mma_stage<NI, 2>(acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, al); break;
-        default: mma_stage<NI, 1>(acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, al); break;
+        case 4: mma_stage<NI, 4, FULL>(acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, kv, fc); break;
+        case 3: mma_stage<NI, 3, FULL>(acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, kv, fc); break;
+        case 2: mma_stage<NI, 2, FULL>(acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, kv, fc); break;
+        default: mma_stage<NI, 1, FULL>(acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, kv, fc); break;
+    }
+}
+template <bool FULL>
+__device__ __forceinline__ void mma_stage_ni(int ni, int nj, double (&acc)[4][4][2], const double* As,
+                                             const double* Bs, int a_off, int a_ks, int a_ms, int b_off, int b_ks,
+                                             int b_ns, int kv, int fc) {
+    switch (ni) {
+        case 4: mma_stage_nj<4, FULL>(nj, acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, kv, fc); break;
+        case 3: mma_stage_nj<3, FULL>(nj, acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, kv, fc); break;
+        case 2: mma_stage_nj<2, FULL>(nj, acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, kv, fc); break;
+        default: mma_stage_nj<1, FULL>(nj, acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, kv, fc); break;
     }
 }
 
-__global__ void __launch_bounds__(NT2, 3)
+__global__ void __launch_bounds__(NT2, CPS)
 seg_gemm_tma_kernel(const Task* __restrict__ tasks, const Seg* __restrict__ segs, const Tile* __restrict__ tiles,
                     int ntiles, int* __restrict__ counter) {
     extern __shared__ __align__(128) double smem[];
@@ -178,6 +211,8 @@ seg_gemm_tma_kernel(const Task* __restrict__ tasks, const Seg* __restrict__ segs
             bool first = true;
             int s = 0, lk = 0;
             if (lastseg >= 1) nxt = sg[1];
+            double ratio = 1.0;                               // != 1 on the first stage of a segment whose alpha differs
+            bool rescale = false;
             do {                                              // one pipeline stage per iteration
                 const int stage = pstep % ST2;
                 mbar_wait(&empty_bar[stage], ((pstep / ST2) & 1) ^ 1);
@@ -196,9 +231,11 @@ seg_gemm_tma_kernel(const Task* __restrict__ tasks, const Seg* __restrict__ segs
                 if (lane == 0) {
                     StageInfo& in = info[stage];
                     in.alpha = compute ? cur.alpha : 0.0;
+                    in.ratio = ratio;
                     in.kv = kv;
                     in.flags = stop ? F_STOP
-                                    : ((compute ? (F_COMPUTE | (cur.flags & 3)) : 0) | (first ? F_FIRST : 0) | (last ? F_LAST : 0));
+                                    : ((compute ? (F_COMPUTE | (cur.flags & 3)) : 0) | (first ? F_FIRST : 0) | (last ? F_LAST : 0) |
+                                       (rescale ? F_RESCALE : 0));
                     if (first && !stop) {
                         TileInfo& ti = tring[tslot];
                         ti.C = tk.C; ti.ident = sg + tk.ngemm; ti.nident = tk.seg_count - tk.ngemm;
@@ -209,24 +246,24 @@ seg_gemm_tma_kernel(const Task* __restrict__ tasks, const Seg* __restrict__ segs
                 }
                 __syncwarp();
                 if (compute) {
-                    const int c2 = (lane & 7) * 2, r0 = lane >> 3;        // LDGSTS: this lane's 16-byte column chunk and first row
+                    const int c2 = (lane % LCPR) * 2, r0 = lane / LCPR;        // LDGSTS: this lane's 16-byte column chunk and first row
                     if (cur.flags & SEG_TRANS_A) {
                         const double* src = cur.A + (size_t)lk * cur.lda + m0;
                         for (int r = lane; r < rowsA; r += 32) bulk_g2s(As + r * LDM, src + (size_t)r * cur.lda, bytesA, &full_bar[stage]);
                     } else if (c2 < kv) {
                         const double* src = cur.A + (size_t)(m0 + r0) * cur.lda + lk + c2;
                         double* dst = As + r0 * LDK + c2;
-                        const size_t step = (size_t)4 * cur.lda;
+                        const size_t step = (size_t)LRS * cur.lda;
 #pragma unroll 4
-                        for (int r = r0; r < mv; r += 4) { ldgsts16(dst, src); dst += 4 * LDK; src += step; }
+                        for (int r = r0; r < mv; r += LRS) { ldgsts16(dst, src); dst += LRS * LDK; src += step; }
                     }
                     if (cur.flags & SEG_TRANS_B) {
                         if (c2 < kv) {
                             const double* src = cur.B + (size_t)(n0 + r0) * cur.ldb + lk + c2;
                             double* dst = Bs + r0 * LDK + c2;
-                            const size_t step = (size_t)4 * cur.ldb;
+                            const size_t step = (size_t)LRS * cur.ldb;
 #pragma unroll 4
-                            for (int r = r0; r < nv; r += 4) { ldgsts16(dst, src); dst += 4 * LDK; src += step; }
+                            for (int r = r0; r < nv; r += LRS) { ldgsts16(dst, src); dst += LRS * LDK; src += step; }
                         }
                     } else {
                         const double* src = cur.B + (size_t)lk * cur.ldb + n0;
@@ -236,8 +273,12 @@ seg_gemm_tma_kernel(const Task* __restrict__ tasks, const Seg* __restrict__ segs
                     if (lk >= cur.K) {                                // next segment: already in registers
                         lk = 0;
                         ++s;
+                        rescale = (s <= lastseg) && (nxt.alpha != cur.alpha);
+                        if (rescale) ratio = cur.alpha / nxt.alpha;   // segments with alpha == 0 are dropped by the host
                         cur = nxt;
                         if (s + 1 <= lastseg) nxt = sg[s + 1];
+                    } else {
+                        rescale = false;
                     }
                 }
                 ldgsts_arrive_noinc(&full_bar[stage]);                // fires when this lane's LDGSTS of the stage have landed
@@ -277,8 +318,15 @@ seg_gemm_tma_kernel(const Task* __restrict__ tasks, const Seg* __restrict__ segs
 #pragma unroll
                 for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
         }
+        const double al = in.alpha;                         // read before the stage is released
+        if (fl & F_RESCALE) {                                // a new alpha: acc holds sum / alpha_prev -> sum / alpha
+            const double r = in.ratio;
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) { acc[i][j][0] *= r; acc[i][j][1] *= r; }
+        }
         if (fl & F_COMPUTE) {
-            const double al = in.alpha;
             const int kv = in.kv;
             const double* As = smem + stage * STAGE_DOUBLES;
             const double* Bs = As + PANEL;
@@ -291,31 +339,9 @@ seg_gemm_tma_kernel(const Task* __restrict__ tasks, const Seg* __restrict__ segs
             if (ni == 0 || nj == 0) {
                 // nothing to do for this warp in this tile
             } else if (kv == BK) {
-                switch (ni) {
-                    case 4: mma_stage_nj<4>(nj, acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, al); break;
-                    case 3: mma_stage_nj<3>(nj, acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, al); break;
-                    case 2: mma_stage_nj<2>(nj, acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, al); break;
-                    default: mma_stage_nj<1>(nj, acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, al); break;
-                }
-            } else {                                         // ragged K tail (masked in registers; once per segment)
-#pragma unroll
-                for (int kk = 0; kk < BK; kk += 4) {
-                    if (kk < kv) {
-                        const bool ok = kk + fc < kv;
-                        double a[4], b[4];
-#pragma unroll
-                        for (int i = 0; i < 4; ++i) { const double v = As[a_off + kk * a_ks + 8 * i * a_ms]; a[i] = ok ? al * v : 0.0; }
-#pragma unroll
-                        for (int j = 0; j < 4; ++j) { const double v = Bs[b_off + kk * b_ks + 8 * j * b_ns]; b[j] = ok ? v : 0.0; }
-#pragma unroll
-                        for (int i = 0; i < 4; ++i)
-                            if (i < ni) {
-#pragma unroll
-                                for (int j = 0; j < 4; ++j)
-                                    if (j < nj) dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
-                            }
-                    }
-                }
+                mma_stage_ni<true>(ni, nj, acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, kv, fc);
+            } else {                                         // ragged K tail of a segment
+                mma_stage_ni<false>(ni, nj, acc, As, Bs, a_off, a_ks, a_ms, b_off, b_ks, b_ns, kv, fc);
             }
         }
         __syncwarp();
@@ -336,7 +362,7 @@ seg_gemm_tma_kernel(const Task* __restrict__ tasks, const Seg* __restrict__ segs
                 for (int j = 0; j < 4; ++j) {
                     const int col = tn0 + wn + 8 * j + 2 * fc;
                     if (j >= nj || col >= tn0 + tnv) continue;
-                    double v0 = acc[i][j][0], v1 = acc[i][j][1];
+                    double v0 = al * acc[i][j][0], v1 = al * acc[i][j][1];
                     const bool two = (col + 1 < tn0 + tnv);
                     for (int s = 0; s < tnident; ++s) {
                         const double* ap = tident[s].A + (size_t)row * tident[s].lda + col;
