@@ -39,6 +39,9 @@ void Engine::prepare_bond(int i) {
 }
 HeffPlan::~HeffPlan() {
     if (X) X->drop_temps();
+    for (cudaEvent_t e : ev_p1) cudaEventDestroy(e);
+    for (cudaEvent_t e : ev_p2) cudaEventDestroy(e);
+    if (ev_in) cudaEventDestroy(ev_in);
 }
 
 }  // namespace dmrg
@@ -104,6 +107,7 @@ int dmrg_create(dmrg_ctx** out, int k, int n_elec, int two_sz, const double* h, 
         if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= eng.opt.device_id) { delete ctx; return DMRG_ECUDA; }
         cuda_check(cudaSetDevice(eng.opt.device_id), "cudaSetDevice");
         cuda_check(cudaStreamCreateWithFlags(&eng.stream, cudaStreamNonBlocking), "cudaStreamCreate");
+        cuda_check(cudaStreamCreateWithFlags(&eng.stream2, cudaStreamNonBlocking), "cudaStreamCreate");
         eng.k = k; eng.n_elec = n_elec; eng.two_sz = two_sz;
         eng.bsw = (k >= 3) ? (k - 3) / 2 : -1;
         eng.ham.k = k;
@@ -129,6 +133,7 @@ int dmrg_destroy(dmrg_ctx* ctx) {
     eng.mps.sites.clear();
     if (eng.svd) svd_destroy(eng.svd);
     if (eng.stream) cudaStreamDestroy(eng.stream);
+    if (eng.stream2) cudaStreamDestroy(eng.stream2);
     delete ctx;
     return DMRG_OK;
 }

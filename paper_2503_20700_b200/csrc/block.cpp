@@ -144,6 +144,19 @@ void finalize(GemmBatch& b, GemmLaunch& out, Engine& eng) {
                 tw.push_back((weight[t] + 16.0) * ((mv + 7) / 8) * ((nv + 7) / 8));
             }
     }
+    if (eng.trace) {                                           // flop and stage histogram by fragments of the busiest warp
+        double hf[17] = {0}, hs[17] = {0}, tf = 0, ts = 0;
+        for (size_t j = 0; j < raw.size(); ++j) {
+            const int fm = (raw[j].mv + 7) / 8, fn = (raw[j].nv + 7) / 8, c = ((fm + 1) / 2) * ((fn + 1) / 2);
+            const double kk = weight[raw[j].task];
+            hf[c] += 2.0 * kk * raw[j].mv * raw[j].nv; tf += 2.0 * kk * raw[j].mv * raw[j].nv;
+            hs[c] += kk / 16.0; ts += kk / 16.0;
+        }
+        std::fprintf(stderr, "[dmrg trace] tiles=%zu flops%%/stages%% by max warp fragments:", raw.size());
+        for (int c = 1; c <= 16; ++c)
+            if (hs[c] > 0) std::fprintf(stderr, " %d:%.1f/%.1f", c, 100.0 * hf[c] / tf, 100.0 * hs[c] / ts);
+        std::fprintf(stderr, "\n");
+    }
     std::vector<int> order(raw.size());
     for (size_t j = 0; j < raw.size(); ++j) order[j] = (int)j;
     std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return tw[x] > tw[y]; });
@@ -157,20 +170,21 @@ void finalize(GemmBatch& b, GemmLaunch& out, Engine& eng) {
     out.flops = b.flops;
     cuda_check(cudaStreamSynchronize(eng.stream), "descriptor upload");   // host vectors die after this call
 }
-void run(const GemmLaunch& l, Engine& eng) {
+void run(const GemmLaunch& l, Engine& eng, cudaStream_t st) {
     if (l.ntiles == 0) return;
+    if (!st) st = eng.stream;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (eng.trace) {                                           // DMRG_B200_TRACE=1: per-launch device time on stderr
         cudaEventCreate(&e0); cudaEventCreate(&e1);
-        cudaEventRecord(e0, eng.stream);
+        cudaEventRecord(e0, st);
     }
     if (l.aligned && !eng.force_generic_gemm)
-        launch_seg_gemm_tma(l.tasks.p, l.segs.p, l.tiles.p, l.ntiles, l.counter.p, eng.stream);
+        launch_seg_gemm_tma(l.tasks.p, l.segs.p, l.tiles.p, l.ntiles, l.counter.p, st);
     else
-        launch_seg_gemm(l.tasks.p, l.segs.p, l.tiles.p, l.ntiles, eng.stream);
+        launch_seg_gemm(l.tasks.p, l.segs.p, l.tiles.p, l.ntiles, st);
     eng.launches++;
     if (eng.trace) {
-        cudaEventRecord(e1, eng.stream);
+        cudaEventRecord(e1, st);
         cudaEventSynchronize(e1);
         float ms = 0.f;
         cudaEventElapsedTime(&ms, e0, e1);

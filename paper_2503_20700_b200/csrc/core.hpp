@@ -90,7 +90,7 @@ struct GemmLaunch {                               // device-resident descriptors
 };
 struct Engine;
 void finalize(GemmBatch& b, GemmLaunch& out, Engine& eng);   // sort segs by task, build tiles, upload
-void run(const GemmLaunch& l, Engine& eng);
+void run(const GemmLaunch& l, Engine& eng, cudaStream_t st = nullptr);   // st: stream override (default eng.stream)
 void run_once(GemmBatch& b, Engine& eng);                    // finalize + run + release (synchronises)
 
 // ---- operator storage ----------------------------------------------------------------------------------------------
@@ -167,7 +167,7 @@ struct HeffPlan {
     int64_t nnz = 0;
     struct Chunk { GemmLaunch p1, p2; };
     std::vector<Chunk> chunks;
-    DevVec<double> T, xbuf, ybuf, xpad;           // xpad: x with even leading dimensions, 16-byte aligned blocks
+    DevVec<double> T, T2, xbuf, ybuf, xpad;       // T / T2: intermediates of even / odd chunks (double buffered)           // xpad: x with even leading dimensions, 16-byte aligned blocks
     int64_t nnz_pad = 0;
     DevVec<int64_t> blk_poff;
     DevVec<DiagItem> diag_items;
@@ -177,6 +177,8 @@ struct HeffPlan {
     double f_alg = 0, f_exec = 0, b_alg = 0;
     int64_t nterms = 0, ngemm = 0;
     Block* X = nullptr;                           // block carrying temporaries
+    std::vector<cudaEvent_t> ev_p1, ev_p2;        // per chunk: phase 1 done / phase 2 done
+    cudaEvent_t ev_in = nullptr;                  // x is ready on the main stream
     ~HeffPlan();                                  // drops the temporaries on X
 };
 void psi_layout(const Basis& bl, const Basis& br, std::vector<PsiBlock>& layout, std::vector<int>& lookup,
@@ -205,6 +207,7 @@ struct Engine {
     Options opt;
     int k = 0, n_elec = 0, two_sz = 0, bsw = 0;
     cudaStream_t stream = nullptr;                // the library's own stream
+    cudaStream_t stream2 = nullptr;               // second stream: phase 2 of H_eff psi runs beside the next chunk's phase 1
     MPS mps;
     bool have_mps = false;
     std::map<int, std::unique_ptr<Block>> L, R;   // by bond

@@ -206,11 +206,25 @@ std::unique_ptr<HeffPlan> build_heff(const Ham& ham, Block& LB, Block& RB, int i
         }
     }
     // ---- materialise: allocate T, patch offsets into addresses, upload ------------------------------------------------
-    p.T.alloc((size_t)std::max<int64_t>(t_max, 2));
-    cuda_check(cudaMemsetAsync(p.T.p, 0, (size_t)std::max<int64_t>(t_max, 2) * 8, eng.stream), "memset");   // finite pads
-    for (auto& pc : patchC) builds[pc.chunk].p1.tasks[pc.index].C = p.T.p + pc.off;
-    for (auto& pa : patchA) builds[pa.chunk].p2.segs[pa.index].A = p.T.p + pa.off;
-    for (auto& pb : patchB) builds[pb.chunk].p2.segs[pb.index].B = p.T.p + pb.off;
+    // two buffers: even chunks use T, odd chunks T2, so phase 1 of chunk c+1 can run beside phase 2 of chunk c
+    const size_t tsz = (size_t)std::max<int64_t>(t_max, 2);
+    p.T.alloc(tsz);
+    cuda_check(cudaMemsetAsync(p.T.p, 0, tsz * 8, eng.stream), "memset");   // finite pads
+    if (builds.size() > 1) {
+        p.T2.alloc(tsz);
+        cuda_check(cudaMemsetAsync(p.T2.p, 0, tsz * 8, eng.stream), "memset");
+    }
+    auto tbase = [&](int chunk) { return (chunk & 1) ? p.T2.p : p.T.p; };
+    for (auto& pc : patchC) builds[pc.chunk].p1.tasks[pc.index].C = tbase(pc.chunk) + pc.off;
+    for (auto& pa : patchA) builds[pa.chunk].p2.segs[pa.index].A = tbase(pa.chunk) + pa.off;
+    for (auto& pb : patchB) builds[pb.chunk].p2.segs[pb.index].B = tbase(pb.chunk) + pb.off;
+    p.ev_p1.resize(builds.size());
+    p.ev_p2.resize(builds.size());
+    for (size_t c = 0; c < builds.size(); ++c) {
+        cuda_check(cudaEventCreateWithFlags(&p.ev_p1[c], cudaEventDisableTiming), "event");
+        cuda_check(cudaEventCreateWithFlags(&p.ev_p2[c], cudaEventDisableTiming), "event");
+    }
+    cuda_check(cudaEventCreateWithFlags(&p.ev_in, cudaEventDisableTiming), "event");
     p.chunks.resize(builds.size());
     for (size_t c = 0; c < builds.size(); ++c) {
         p.f_exec += builds[c].p1.flops + builds[c].p2.flops;
@@ -243,9 +257,24 @@ void heff_apply(HeffPlan& p, const double* x_dev, double* y_dev, Engine& eng) {
     // x (packed exchange layout) -> padded, aligned copy read by the GEMM kernel
     launch_pad_blocks(p.xpad.p, x_dev, (int)p.layout.size(), p.blk_poff.p, p.blk_off.p, p.blk_rows.p, p.blk_cols.p, eng.stream);
     eng.launches++;
-    for (auto& c : p.chunks) {
-        run(c.p1, eng);
-        run(c.p2, eng);
+    // Software pipeline over the chunks on two streams: phase 1 (T = O X) of chunk c+1 fills the SMs that the tail of
+    // phase 2 (Y += T O^T) of chunk c leaves idle.  Phase 2 launches stay in chunk order on one stream, so the
+    // accumulation order into y is fixed (bit-reproducible); T is double buffered (chunk parity).
+    const int nc = (int)p.chunks.size();
+    if (nc == 1 || eng.trace) {
+        for (auto& c : p.chunks) { run(c.p1, eng); run(c.p2, eng); }
+    } else {
+        cuda_check(cudaEventRecord(p.ev_in, eng.stream), "event record");
+        cuda_check(cudaStreamWaitEvent(eng.stream2, p.ev_in, 0), "stream wait");
+        for (int c = 0; c < nc; ++c) {
+            if (c >= 2) cuda_check(cudaStreamWaitEvent(eng.stream, p.ev_p2[c - 2], 0), "stream wait");   // T buffer free
+            run(p.chunks[c].p1, eng, eng.stream);
+            cuda_check(cudaEventRecord(p.ev_p1[c], eng.stream), "event record");
+            cuda_check(cudaStreamWaitEvent(eng.stream2, p.ev_p1[c], 0), "stream wait");
+            run(p.chunks[c].p2, eng, eng.stream2);
+            cuda_check(cudaEventRecord(p.ev_p2[c], eng.stream2), "event record");
+        }
+        cuda_check(cudaStreamWaitEvent(eng.stream, p.ev_p2[nc - 1], 0), "stream wait");
     }
     if (y_dev != p.ybuf.p)
         cuda_check(cudaMemcpyAsync(y_dev, p.ybuf.p, (size_t)p.nnz * 8, cudaMemcpyDeviceToDevice, eng.stream), "y copy");
