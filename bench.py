@@ -41,7 +41,7 @@ def parse_args():
     ap.add_argument("--config", type=int, default=4, help="BASELINE config 1..5 (default 4: the metric's workload)")
     ap.add_argument("--D", type=int, default=0, help="bond dimension override (0 = the config's)")
     ap.add_argument("--bond", type=int, default=-1, help="two-site bond (default mid-chain k/2-1)")
-    ap.add_argument("--extras", type=int, default=1, help="1: also time a small sweep + RDM (config 1)")
+    ap.add_argument("--extras", type=int, default=1, help="1: also time sweeps + RDM on config 1; 2: on configs 1-3")
     ap.add_argument("--cpu-baseline", type=int, default=1)
     ap.add_argument("--sample-config", type=int, default=2, help="config of the oracle's bounded sample")
     ap.add_argument("--sample-D", type=int, default=96)
@@ -211,36 +211,47 @@ def run_reference(args):
     print(json.dumps(line))
 
 
-def time_small_extras(P, torch):
-    """Seconds per sweep and 1-/2-RDM time on BASELINE config 1 (D = 64): the remaining rows of the hot path
-    (a1, a3, a4, a5, a6) exercised end to end in the same run."""
+def time_small_extras(P, torch, peaks, level):
+    """Seconds per sweep and 1-/2-RDM time on BASELINE configs 1 (D = 64), 2 (D = 512) and 3 (D = 1024): the remaining
+    rows of the hot path (a1, a3, a4, a5, a6) exercised end to end in the same run.  level 1: config 1 only; 2: configs
+    1-3 with one sweep each (from a seeded random MPS, so bond dimensions are saturated from the start)."""
     from synth import make_config, random_mps, mps_to_blob_arrays
     out = {}
-    cfg = make_config(1)
-    k, n = cfg["k"], cfg["n_elec"]
-    mps = random_mps(k, n, 0, 64, seed=cfg["seed"] + 1000, gauge="R")
-    ctx = P.dmrg_create(k, n, 0, cfg["h"], cfg["eri"])
-    try:
-        P.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, 0)
-        secs, e = [], None
-        for _ in range(3):
-            r = P.dmrg_sweep(ctx, 64, k)
-            secs.append(r["seconds"])
-            e = r["energy_last"]
-        out["sweep"] = {"workload": cfg["name"] + " D=64", "s_per_sweep": secs, "energy_last_eh": e + cfg["e_core"],
-                        "matvecs_last_sweep": int(sum(b["n_matvec"] for b in r["bonds"]))}
+    for cid, nsweep in ((1, 3), (2, 1), (3, 1))[: (1 if level == 1 else 3)]:
+        cfg = make_config(cid)
+        k, n, D = cfg["k"], cfg["n_elec"], cfg["D"]
+        mps = random_mps(k, n, 0, D, seed=cfg["seed"] + 1000, gauge="R")
+        ctx = P.dmrg_create(k, n, 0, cfg["h"], cfg["eri"])
+        rec = {"workload": "%s D=%d" % (cfg["name"], D)}
         try:
-            t0 = time.perf_counter()
-            g, G = P.dmrg_rdm12(ctx, k, True)
-            torch.cuda.synchronize()
-            st = P.dmrg_rdm_stats(ctx)
-            out["rdm12"] = {"workload": cfg["name"] + " D=64", "seconds": time.perf_counter() - t0,
-                            "device_seconds": st["seconds"], "trace_gamma": float(np.trace(g)),
-                            "gbytes_streamed": st["bytes_streamed"] / 1e9}
-        except P.binding.DmrgError as ex:
-            out["rdm12"] = {"error": str(ex)}
-    finally:
-        P.dmrg_destroy(ctx)
+            P.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, 0)
+            secs, e, r = [], None, None
+            for _ in range(nsweep):
+                r = P.dmrg_sweep(ctx, D, k)
+                secs.append(r["seconds"])
+                e = r["energy_last"]
+            mv = int(sum(b["n_matvec"] for b in r["bonds"]))
+            fl = float(sum(b["n_matvec"] * b["f_alg"] for b in r["bonds"]))
+            tmv = float(sum(b["seconds_matvec"] for b in r["bonds"]))
+            rec["sweep"] = {"s_per_sweep": secs, "energy_last_eh": e + cfg["e_core"], "matvecs_last_sweep": mv,
+                            "matvec_seconds_last_sweep": tmv, "matvec_f_alg_last_sweep": fl,
+                            "matvec_tflops_last_sweep": fl / tmv / 1e12 if tmv > 0 else None,
+                            "max_kept": int(max(b["kept"] for b in r["bonds"]))}
+            try:
+                t0 = time.perf_counter()
+                g, G = P.dmrg_rdm12(ctx, k, True)
+                torch.cuda.synchronize()
+                st = P.dmrg_rdm_stats(ctx)
+                gbs = st["bytes_streamed"] / st["stream_seconds"] / 1e9 if st["stream_seconds"] > 0 else None
+                rec["rdm12"] = {"seconds": time.perf_counter() - t0, "device_seconds": st["seconds"],
+                                "trace_gamma": float(np.trace(g)), "gbytes_streamed": st["bytes_streamed"] / 1e9,
+                                "stream_seconds": st["stream_seconds"], "stream_gbs": gbs,
+                                "stream_frac_of_hbm": gbs / peaks["hbm"] if gbs else None, "flops": st["flops"]}
+            except P.binding.DmrgError as ex:
+                rec["rdm12"] = {"error": str(ex)}
+        finally:
+            P.dmrg_destroy(ctx)
+        out["config%d" % cid] = rec
     return out
 
 
@@ -362,7 +373,7 @@ def run_ours(args):
         line["fp64_probe"] = pr
         roof["frac_of_dmma_probe"] = achieved / pr["dmma_regs"]["tflops"]
     if args.extras:
-        line["extras"] = time_small_extras(P, torch)
+        line["extras"] = time_small_extras(P, torch, peaks, args.extras)
     if args.cpu_baseline and world == 1:
         v, info = oracle_sample(args, 3, 1)
         line["cpu_baseline"] = dict(info, value=v, unit=UNIT)

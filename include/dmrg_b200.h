@@ -136,8 +136,11 @@ int dmrg_sweep(dmrg_ctx* ctx, int D, dmrg_sweep_result* result, dmrg_bond_record
  * device per `where`. */
 int dmrg_rdm12(dmrg_ctx* ctx, double* gamma, double* Gamma, int where, void* cuda_stream);
 
-/* Timing / accounting of the last dmrg_rdm12 call: device seconds, bytes of operator storage streamed, flops. */
-int dmrg_rdm_stats(dmrg_ctx* ctx, double* seconds, double* bytes_streamed, double* flops);
+/* Timing / accounting of the last dmrg_rdm12 call: seconds of the whole pass, bytes of operator storage streamed by
+ * the accumulation kernels (E = Stack M^T: every stored operator once per centre, plus the M vectors), all flops, and
+ * the device seconds (CUDA events) of those accumulation kernels alone, so that bytes_streamed / stream_seconds is
+ * their achieved HBM rate.  Any output pointer may be null. */
+int dmrg_rdm_stats(dmrg_ctx* ctx, double* seconds, double* bytes_streamed, double* flops, double* stream_seconds);
 
 /* Number of kernels this library launched on the context since creation (bench.py's gpu_launches). */
 int64_t dmrg_launch_count(const dmrg_ctx* ctx);

@@ -201,9 +201,9 @@ def dmrg_rdm12(ctx, k, want_2rdm=True):
 
 
 def dmrg_rdm_stats(ctx):
-    s, b, f = C.c_double(), C.c_double(), C.c_double()
-    _check(ctx, lib.dmrg_rdm_stats(ctx, C.byref(s), C.byref(b), C.byref(f)))
-    return dict(seconds=s.value, bytes_streamed=b.value, flops=f.value)
+    s, b, f, t = C.c_double(), C.c_double(), C.c_double(), C.c_double()
+    _check(ctx, lib.dmrg_rdm_stats(ctx, C.byref(s), C.byref(b), C.byref(f), C.byref(t)))
+    return dict(seconds=s.value, bytes_streamed=b.value, flops=f.value, stream_seconds=t.value)
 
 
 def dmrg_launch_count(ctx):

@@ -378,11 +378,12 @@ int dmrg_rdm12(dmrg_ctx* ctx, double* gamma, double* Gamma, int where, void* cud
     API_END
 }
 
-int dmrg_rdm_stats(dmrg_ctx* ctx, double* seconds, double* bytes_streamed, double* flops) {
+int dmrg_rdm_stats(dmrg_ctx* ctx, double* seconds, double* bytes_streamed, double* flops, double* stream_seconds) {
     API_BEGIN(ctx)
     if (seconds) *seconds = eng.rdm_seconds;
     if (bytes_streamed) *bytes_streamed = eng.rdm_bytes;
     if (flops) *flops = eng.rdm_flops;
+    if (stream_seconds) *stream_seconds = eng.rdm_stream_ms * 1e-3;
     return DMRG_OK;
     API_END
 }

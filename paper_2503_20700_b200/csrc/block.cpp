@@ -201,6 +201,24 @@ void run_once(GemmBatch& b, Engine& eng) {
     cuda_check(cudaStreamSynchronize(eng.stream), "grouped GEMM");
     b = GemmBatch();
 }
+double run_once_ms(GemmBatch& b, Engine& eng) {
+    if (b.tasks.empty()) return 0.0;
+    GemmLaunch l;
+    finalize(b, l, eng);
+    cudaEvent_t e0, e1;
+    cuda_check(cudaEventCreate(&e0), "event");
+    cuda_check(cudaEventCreate(&e1), "event");
+    cudaEventRecord(e0, eng.stream);
+    run(l, eng);
+    cudaEventRecord(e1, eng.stream);
+    cuda_check(cudaStreamSynchronize(eng.stream), "grouped GEMM");
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    b = GemmBatch();
+    return (double)ms;
+}
 
 // ---------------------------------------------------------------------------------------------------------------
 // Block

@@ -92,6 +92,7 @@ struct Engine;
 void finalize(GemmBatch& b, GemmLaunch& out, Engine& eng);   // sort segs by task, build tiles, upload
 void run(const GemmLaunch& l, Engine& eng, cudaStream_t st = nullptr);   // st: stream override (default eng.stream)
 void run_once(GemmBatch& b, Engine& eng);                    // finalize + run + release (synchronises)
+double run_once_ms(GemmBatch& b, Engine& eng);               // same, returns the kernel's device time (CUDA events)
 
 // ---- operator storage ----------------------------------------------------------------------------------------------
 struct OpClass {                                  // block structure shared by all operators with one label shift
@@ -216,6 +217,8 @@ struct Engine {
     std::string last_error;
     SvdWork* svd = nullptr;
     double rdm_seconds = 0, rdm_bytes = 0, rdm_flops = 0;
+    double t_plan = 0, t_davidson = 0, t_split = 0, t_grow = 0, t_matvec = 0;   // phase seconds of the last sweep
+    double rdm_stream_ms = 0;                     // device time of the operator-streaming kernels (E = Stack M^T) alone
     bool keep_env_stack = true;
     bool sweep_ready = false;                     // environments consistent with the sweep position
     bool trace = false;                           // DMRG_B200_TRACE=1: print every grouped-GEMM launch's device time

@@ -351,7 +351,7 @@ void evaluate_group(CentreCtx& cx, ColGroup& g, const std::vector<int>& stacks, 
             }
             eng.rdm_flops += gb.flops;
             eng.rdm_bytes += 8.0 * ((double)nrows * ld + (double)nc * ld);
-            run_once(gb, eng);
+            eng.rdm_stream_ms += run_once_ms(gb, eng);
             run_once(red, eng);
             std::vector<double>& E = out.E[s];
             cuda_check(cudaMemcpy2DAsync(E.data() + c0, (size_t)ncol * 8, Ed.p, (size_t)nc * 8, (size_t)nc * 8, nrows,
@@ -375,7 +375,7 @@ void rdm12(Engine& eng, double* gamma, double* Gamma) {
     for (int p = 1; p < k; ++p)
         if (mps.sites[p].gauge != 'R')
             throw Error(-2, "rdm12: the MPS must be right-canonical with its centre on site 0 (as imported or as left by dmrg_sweep)");
-    eng.rdm_bytes = 0; eng.rdm_flops = 0;
+    eng.rdm_bytes = 0; eng.rdm_flops = 0; eng.rdm_stream_ms = 0;
     std::memset(gamma, 0, sizeof(double) * (size_t)k * k);
     if (want2) std::memset(Gamma, 0, sizeof(double) * (size_t)k * k * k * k);
     // right blocks with the one-index operators of the sites > c

@@ -3,6 +3,7 @@
 // iteration and the singular values of each bond.
 #include <algorithm>
 #include <chrono>
+#include <cstdio>
 #include <cmath>
 
 #include "core.hpp"
@@ -297,23 +298,31 @@ void split_theta(MPS& mps, int i, const HeffPlan& p, const double* theta, int D,
 // one sweep: forward pass over bonds 0..k-2, backward pass k-2..0 (reading S12)
 // ---------------------------------------------------------------------------------------------------------------
 static BondRecord optimise(Engine& eng, int i, int D, bool forward) {
-    const auto t0 = std::chrono::steady_clock::now();
+    typedef std::chrono::steady_clock clk;
+    auto secs = [](clk::time_point a, clk::time_point b) { return std::chrono::duration<double>(b - a).count(); };
+    const auto t0 = clk::now();
     eng.plan.reset();
     eng.plan = build_heff(eng.ham, *eng.L.at(i), *eng.R.at(i + 2), i, eng);
     HeffPlan& p = *eng.plan;
+    const auto t1 = clk::now();
     DevVec<double> theta;
     theta.alloc((size_t)p.nnz);
     two_site_tensor(eng.mps, i, p, theta.p, eng);
     const DavidsonResult dr = davidson(p, theta.p, eng);
+    const auto t2 = clk::now();
     BondRecord rec;
     rec.bond = i; rec.forward = forward ? 1 : 0;
     rec.energy = dr.theta; rec.residual = dr.residual; rec.n_matvec = dr.n_matvec; rec.converged = dr.converged ? 1 : 0;
     rec.nnz = p.nnz; rec.f_alg = p.f_alg; rec.seconds_matvec = dr.seconds_matvec;
     split_theta(eng.mps, i, p, theta.p, D, forward, eng, rec.trunc_err, rec.kept, rec.nsectors);
+    const auto t3 = clk::now();
     eng.plan.reset();                                          // releases the temporaries before the block grows
     if (forward) eng.L[i + 1] = grow(*eng.L.at(i), eng.ham, eng.mps, eng.mode_L(i + 1), eng);
     else         eng.R[i + 1] = grow(*eng.R.at(i + 2), eng.ham, eng.mps, eng.mode_R(i + 1), eng);
-    rec.seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+    const auto t4 = clk::now();
+    rec.seconds = secs(t0, t4);
+    eng.t_plan += secs(t0, t1); eng.t_davidson += secs(t1, t2); eng.t_split += secs(t2, t3); eng.t_grow += secs(t3, t4);
+    eng.t_matvec += dr.seconds_matvec;
     return rec;
 }
 
@@ -328,9 +337,13 @@ int sweep(Engine& eng, int D, std::vector<BondRecord>& recs, double& seconds) {
         eng.sweep_ready = true;
     }
     recs.clear();
+    eng.t_plan = eng.t_davidson = eng.t_split = eng.t_grow = eng.t_matvec = 0.0;
     for (int i = 0; i <= k - 2; ++i) recs.push_back(optimise(eng, i, D, true));
     for (int i = k - 2; i >= 0; --i) recs.push_back(optimise(eng, i, D, false));
     seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+    if (eng.trace)
+        std::fprintf(stderr, "[dmrg trace] sweep D=%d: %.2f s = plan (block maps) %.2f + davidson %.2f (matvec %.2f) + svd/split %.2f + renormalise %.2f\n",
+                     D, seconds, eng.t_plan, eng.t_davidson, eng.t_matvec, eng.t_split, eng.t_grow);
     int warnings = 0;
     for (const BondRecord& r : recs) if (!r.converged) ++warnings;
     return warnings;
