@@ -116,6 +116,7 @@ int dmrg_create(dmrg_ctx** out, int k, int n_elec, int two_sz, const double* h, 
         eng.svd = svd_create(eng.stream);
         { const char* g = std::getenv("DMRG_B200_GENERIC_GEMM"); eng.force_generic_gemm = g && g[0] == '1'; }
         { const char* g = std::getenv("DMRG_B200_TRACE"); eng.trace = g && g[0] == '1'; }
+        { const char* g = std::getenv("DMRG_B200_HOST_MAPS"); eng.host_maps = g && g[0] == '1'; }
     } catch (...) {
         delete ctx;
         return DMRG_ECUDA;

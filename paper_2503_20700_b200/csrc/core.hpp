@@ -221,6 +221,7 @@ struct Engine {
     double rdm_stream_ms = 0;                     // device time of the operator-streaming kernels (E = Stack M^T) alone
     bool keep_env_stack = true;
     bool sweep_ready = false;                     // environments consistent with the sweep position
+    bool host_maps = false;                       // DMRG_B200_HOST_MAPS=1: build the H_eff block maps on the host (A/B testing)
     bool trace = false;                           // DMRG_B200_TRACE=1: print every grouped-GEMM launch's device time
     bool force_generic_gemm = false;              // DMRG_B200_GENERIC_GEMM=1: always the cp.async kernel (A/B testing)
     char mode_L(int b) const { return b <= bsw ? 'N' : 'C'; }

@@ -11,6 +11,7 @@
 #include <cassert>
 
 #include "core.hpp"
+#include "maps.hpp"
 
 namespace dmrg {
 
@@ -83,6 +84,150 @@ int64_t Engine::t_capacity() const {
     return std::max(lo, std::min(cap, hi));
 }
 
+namespace {
+
+template <class T>
+T* upload_vec(const std::vector<T>& v, std::vector<void*>& keep, cudaStream_t st) {
+    T* d = (T*)dev_alloc(std::max<size_t>(v.size(), 1) * sizeof(T));
+    keep.push_back(d);
+    if (!v.empty()) cuda_check(cudaMemcpyAsync(d, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice, st), "upload");
+    return d;
+}
+
+// flattened quantum-number maps of every operator class of a block
+MapSide upload_side(const Block& B, std::vector<void*>& keep, cudaStream_t st) {
+    const int nsec = (int)B.basis.size(), ncls = (int)B.classes.size();
+    std::vector<int> out((size_t)ncls * nsec, -1), inv((size_t)ncls * nsec, -1), dim(nsec);
+    std::vector<int64_t> off((size_t)ncls * nsec, 0);
+    for (int c = 0; c < ncls; ++c)
+        for (int a = 0; a < nsec; ++a) {
+            out[(size_t)c * nsec + a] = B.classes[c].out[a];
+            inv[(size_t)c * nsec + a] = B.classes[c].inv[a];
+            off[(size_t)c * nsec + a] = B.classes[c].off[a];
+        }
+    for (int a = 0; a < nsec; ++a) dim[a] = B.basis[a].d;
+    MapSide sd;
+    sd.out = upload_vec(out, keep, st); sd.inv = upload_vec(inv, keep, st); sd.off = upload_vec(off, keep, st);
+    sd.dim = upload_vec(dim, keep, st); sd.nsec = nsec; sd.pad = 0;
+    return sd;
+}
+
+void adopt(GemmLaunch& l, Task* tasks, int nt, Seg* segs, int ns, Tile* tiles, int ntiles, double flops) {
+    l.tasks.p = tasks; l.tasks.n = (size_t)nt;
+    l.segs.p = segs; l.segs.n = (size_t)ns;
+    l.tiles.p = tiles; l.tiles.n = (size_t)ntiles;
+    l.ntiles = ntiles; l.flops = flops; l.aligned = true;     // every operand of H_eff psi is 16-byte aligned with an even ld
+    if (!l.counter.p) l.counter.alloc(1);
+}
+
+}  // namespace
+
+// Device-built block maps: the host uploads O(terms + classes x sectors) integers, the kernels of
+// heff_maps.cu enumerate everything that scales as terms x blocks.
+static void build_maps_device(HeffPlan& p, const std::vector<NTerm>& terms, Block& LB, Block& RB, const Dot& dot,
+                              Engine& eng) {
+    cudaStream_t st = eng.stream;
+    std::vector<void*> keep;                                   // tables only needed while building
+    struct Guard { std::vector<void*>& k; ~Guard() { for (void* q : k) dev_free(q); } } guard{keep};
+    const int nblk = (int)p.layout.size();
+    // ---- tables ----------------------------------------------------------------------------------------------------------
+    std::vector<MapBlock> blocks(nblk);
+    for (int b = 0; b < nblk; ++b) {
+        const PsiBlock& q = p.layout[b];
+        blocks[b] = {q.l, q.ab, q.r, q.rows, q.cols, 0, q.off, q.poff};
+    }
+    std::vector<MapOp> opsL, opsR;
+    std::vector<int> refclsL, refclsR;
+    std::unordered_map<uint64_t, int> idxL, idxR, refL, refR;
+    auto op_index = [&](Block& B, const Label& lab, bool trans, std::vector<MapOp>& ops, std::vector<int>& refcls,
+                        std::unordered_map<uint64_t, int>& idx, std::unordered_map<uint64_t, int>& ref) {
+        const uint64_t k1 = (uint64_t)lab.key() * 2 + (trans ? 1 : 0);
+        auto it = idx.find(k1);
+        if (it != idx.end()) return it->second;
+        const OpRef& r = B.get(lab);
+        auto ir = ref.find(lab.key());
+        if (ir == ref.end()) { ir = ref.emplace(lab.key(), (int)refcls.size()).first; refcls.push_back(r.cls); }
+        ops.push_back({r.ptr, r.cls, trans ? 1 : 0, ir->second, 0});
+        idx.emplace(k1, (int)ops.size() - 1);
+        return (int)ops.size() - 1;
+    };
+    std::vector<double> dmtab;
+    std::map<std::vector<double>, int> dmidx;
+    std::vector<MapTerm> mt, mt_ident;
+    for (const NTerm& nt : terms) {
+        if (nt.coef == 0.0) continue;
+        MapTerm t;
+        t.opL = nt.hasL ? op_index(LB, nt.L, nt.transL, opsL, refclsL, idxL, refL) : -1;
+        t.opR = nt.hasR ? op_index(RB, nt.R, nt.transR, opsR, refclsR, idxR, refR) : -1;
+        auto id = dmidx.find(nt.dm.a);
+        if (id == dmidx.end()) {
+            id = dmidx.emplace(nt.dm.a, (int)dmidx.size()).first;
+            dmtab.insert(dmtab.end(), nt.dm.a.begin(), nt.dm.a.end());
+        }
+        t.dm = id->second;
+        t.pd = dot.parity(nt.dm); t.pr = nt.hasR ? KIND_PAR[nt.R.kind] : 0; t.pad = 0; t.coef = nt.coef;
+        (t.opL < 0 && t.opR < 0 ? mt_ident : mt).push_back(t);
+    }
+    mt.insert(mt.end(), mt_ident.begin(), mt_ident.end());     // operator-free terms last: their segments close every task
+    std::vector<int> nL(LB.basis.size());
+    for (size_t l = 0; l < LB.basis.size(); ++l) nL[l] = LB.basis[l].n;
+    MapCtx cx;
+    cx.blocks = upload_vec(blocks, keep, st); cx.lookup = upload_vec(p.lookup, keep, st);
+    cx.terms = upload_vec(mt, keep, st); cx.dm = upload_vec(dmtab, keep, st);
+    cx.opsL = upload_vec(opsL, keep, st); cx.opsR = upload_vec(opsR, keep, st);
+    cx.refclsL = upload_vec(refclsL, keep, st); cx.refclsR = upload_vec(refclsR, keep, st);
+    cx.nL = upload_vec(nL, keep, st); cx.dotqn = upload_vec(dot.qn, keep, st);
+    cx.L = upload_side(LB, keep, st); cx.R = upload_side(RB, keep, st);
+    cx.nblk = nblk; cx.nterm = (int)mt.size(); cx.nopsL = (int)opsL.size(); cx.nopsR = (int)opsR.size();
+    cx.nrefL = (int)refclsL.size(); cx.nrefR = (int)refclsR.size();
+    cx.xpad = p.xpad.p; cx.y = p.ybuf.p;
+    // ---- pass A: accounting, diagonal, per-term intermediate usage -> chunks ---------------------------------------------------
+    MapBuild mb;
+    std::vector<double> usage;
+    maps_usage(cx, usage, mb, dev_alloc, dev_free, st);
+    p.diag_items.p = mb.diag_items; p.diag_items.n = (size_t)std::max(mb.ndiag, 1);
+    p.diag_ptr.p = mb.diag_ptr; p.diag_ptr.n = (size_t)nblk + 1;
+    const int64_t cap = eng.t_capacity();
+    std::vector<int> cbegin(1, 0);
+    double used = 0.0, t_max = 0.0;
+    for (int t = 0; t < cx.nterm; ++t) {
+        if (used > (double)(cap / 2)) { cbegin.push_back(t); used = 0.0; }
+        used += usage[t];
+        t_max = std::max(t_max, used);
+    }
+    cbegin.push_back(cx.nterm);
+    const int nc = (int)cbegin.size() - 1;
+    const size_t tsz = (size_t)std::max<double>(t_max, 2.0);
+    p.T.alloc(tsz);
+    cuda_check(cudaMemsetAsync(p.T.p, 0, tsz * 8, st), "memset");     // finite pads
+    if (nc > 1) { p.T2.alloc(tsz); cuda_check(cudaMemsetAsync(p.T2.p, 0, tsz * 8, st), "memset"); }
+    // ---- pass B: descriptors of every chunk ------------------------------------------------------------------------------------
+    p.chunks.resize(nc);
+    p.ev_p1.resize(nc); p.ev_p2.resize(nc);
+    double ngemm = mb.ngemm;
+    for (int c = 0; c < nc; ++c) {
+        MapChunkOut o;
+        maps_chunk(cx, cbegin[c], cbegin[c + 1], c == 0, (c & 1) ? p.T2.p : p.T.p, o, dev_alloc, dev_free, st);
+        if ((size_t)o.t_doubles > tsz) throw std::logic_error("heff: intermediate buffer bound violated");
+        adopt(p.chunks[c].p1, o.tasks1, o.ntasks1, o.segs1, o.nsegs1, o.tiles1, o.ntiles1, o.flops1);
+        adopt(p.chunks[c].p2, o.tasks2, o.ntasks2, o.segs2, o.nsegs2, o.tiles2, o.ntiles2, o.flops2);
+        p.f_exec += o.flops1 + o.flops2;
+        ngemm += o.ntasks1;
+        cuda_check(cudaEventCreateWithFlags(&p.ev_p1[c], cudaEventDisableTiming), "event");
+        cuda_check(cudaEventCreateWithFlags(&p.ev_p2[c], cudaEventDisableTiming), "event");
+    }
+    cuda_check(cudaEventCreateWithFlags(&p.ev_in, cudaEventDisableTiming), "event");
+    p.f_alg = mb.f_alg; p.ngemm = (int64_t)ngemm;
+    p.b_alg = mb.b_ops + 16.0 * (double)p.nnz;
+    // block tables for the diagonal / padding kernels
+    std::vector<int> rows(nblk), cols(nblk);
+    std::vector<int64_t> offs(nblk), poffs(nblk);
+    for (int b = 0; b < nblk; ++b) { rows[b] = p.layout[b].rows; cols[b] = p.layout[b].cols; offs[b] = p.layout[b].off; poffs[b] = p.layout[b].poff; }
+    p.blk_poff.upload(poffs, st); p.blk_rows.upload(rows, st); p.blk_cols.upload(cols, st); p.blk_off.upload(offs, st);
+    cuda_check(cudaStreamSynchronize(st), "heff maps");
+    cuda_check(cudaGetLastError(), "heff maps kernels");
+}
+
 std::unique_ptr<HeffPlan> build_heff(const Ham& ham, Block& LB, Block& RB, int i, Engine& eng) {
     std::unique_ptr<HeffPlan> pp(new HeffPlan());
     HeffPlan& p = *pp;
@@ -98,7 +243,12 @@ std::unique_ptr<HeffPlan> build_heff(const Ham& ham, Block& LB, Block& RB, int i
     p.xpad.alloc((size_t)std::max<int64_t>(p.nnz_pad, 2));
     cuda_check(cudaMemsetAsync(p.xpad.p, 0, (size_t)std::max<int64_t>(p.nnz_pad, 2) * 8, eng.stream), "memset");
 
-    // ---- enumerate contributions term by term, chunked by the intermediate buffer ---------------------------------
+    if (!eng.host_maps) {                                      // block maps built on the device (heff_maps.cu)
+        build_maps_device(p, terms, LB, RB, dot, eng);
+        return pp;
+    }
+    // ---- host reference builder (DMRG_B200_HOST_MAPS=1; A/B testing of the device builder) ----------------------------
+    // enumerate contributions term by term, chunked by the intermediate buffer
     const int64_t cap = eng.t_capacity();
     int64_t t_max = 0;
     struct ChunkBuild { GemmBatch p1, p2; std::vector<int> task_of; };
