@@ -45,6 +45,7 @@ def parse_args():
     ap.add_argument("--cpu-baseline", type=int, default=1)
     ap.add_argument("--sample-config", type=int, default=2, help="config of the oracle's bounded sample")
     ap.add_argument("--sample-D", type=int, default=96)
+    ap.add_argument("--workspace-gb", type=float, default=0.0, help="intermediate workspace of H_eff psi (0 = library default)")
     ap.add_argument("--probe", type=int, default=1, help="1: run the FP64 ceiling probes (DMMA, DFMA, LDS-fed DMMA, cuBLAS DGEMM)")
     return ap.parse_args()
 
@@ -275,7 +276,8 @@ def run_ours(args):
     t_setup = time.perf_counter()
     cfg, D, i, mps, blob = build_workload(args.config, args.D, args.bond)
     k, n = cfg["k"], cfg["n_elec"]
-    ctx = P.dmrg_create(k, n, 0, cfg["h"], cfg["eri"], keep_env_stack=0, device_id=local_rank)
+    ctx = P.dmrg_create(k, n, 0, cfg["h"], cfg["eri"], keep_env_stack=0, device_id=local_rank,
+                        workspace_bytes=int(args.workspace_gb * (1 << 30)))
     P.dmrg_mps_import(ctx, blob, k, n, 0)
     t_env = time.perf_counter()
     P.dmrg_prepare_bond(ctx, i)                      # renormalisation of both environments + block maps (a1, a5)

@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <chrono>
 #include <cstdio>
+#include <cstdlib>
 #include <cmath>
 
 #include "core.hpp"
@@ -341,7 +342,7 @@ int sweep(Engine& eng, int D, std::vector<BondRecord>& recs, double& seconds) {
     for (int i = 0; i <= k - 2; ++i) recs.push_back(optimise(eng, i, D, true));
     for (int i = k - 2; i >= 0; --i) recs.push_back(optimise(eng, i, D, false));
     seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
-    if (eng.trace)
+    if (eng.trace || std::getenv("DMRG_B200_TIMERS"))
         std::fprintf(stderr, "[dmrg trace] sweep D=%d: %.2f s = plan (block maps) %.2f + davidson %.2f (matvec %.2f) + svd/split %.2f + renormalise %.2f\n",
                      D, seconds, eng.t_plan, eng.t_davidson, eng.t_matvec, eng.t_split, eng.t_grow);
     int warnings = 0;
