@@ -30,6 +30,9 @@ UNIT = "TFLOP/s"
 FP64_FLOP_PER_CLK_SM = 128.0          # DMMA: 64 FP64 FMA / clk / SM
 N_SM = 148
 BF16_NOMINAL_TF = 2250.0
+# dram__bytes_read.sum + dram__bytes_write.sum over the 56 seg_gemm_tma_kernel launches of one H_eff psi at config 4,
+# D = 4096, bond 26, from the ncu capture profiles/r01_step_dram_heff_cfg4.md (same launch configuration as this bench)
+NCU_TRAFFIC_BYTES_PER_STEP_CFG4 = 3.7423e12
 
 
 def parse_args():
@@ -346,7 +349,9 @@ def run_ours(args):
     t_byte = st["b_alg"] / (peaks["hbm"] * 1e9)
     achieved = st["f_exec"] / (ms_per_step * 1e-3) / 1e12
     roof = {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-            "traffic": None, "kernel": "seg_gemm_kernel (FP64 DMMA.8x8x4)", "launches_per_step": launches / args.steps,
+            "traffic": NCU_TRAFFIC_BYTES_PER_STEP_CFG4 if (args.config == 4 and D == 4096 and i == k // 2 - 1) else None,
+            "traffic_note": "bytes per step (all launches of one H_eff psi), like achieved; ncu, profiles/r01_step_dram_heff_cfg4.md",
+            "kernel": "seg_gemm_tma_kernel (FP64 DMMA.8x8x4, bulk-copy fed)", "launches_per_step": launches / args.steps,
             "peak_source": "%s bf16 burst %.1f TF x nominal FP64/bf16 ratio (%.1f / %.0f TF); FP64 nominal = 148 SM x "
                            "128 flop/clk x %.0f MHz" % (peaks["src"], peaks["bf16"], nominal, BF16_NOMINAL_TF, peaks["sm_max"]),
             "peak_nominal_fp64": nominal, "frac_of_nominal": achieved / nominal,
