@@ -168,6 +168,9 @@ struct HeffPlan {
     int64_t nnz = 0;
     struct Chunk { GemmLaunch p1, p2; };
     std::vector<Chunk> chunks;
+    int split = 1;                                // split-K parts of phase 2 (device-built maps): parts >= 1 go to ypart
+    DevVec<double> ypart;                         // (split - 1) x nnz partial sums
+    GemmLaunch reduce;                            // y += sum of the partial sums, in part order
     DevVec<double> T, T2, xbuf, ybuf, xpad;       // T / T2: intermediates of even / odd chunks (double buffered)           // xpad: x with even leading dimensions, 16-byte aligned blocks
     int64_t nnz_pad = 0;
     DevVec<int64_t> blk_poff;

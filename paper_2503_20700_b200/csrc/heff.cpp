@@ -9,6 +9,7 @@
 // atomics, fixed summation order.  Terms are processed in chunks bounded by the intermediate buffer.
 #include <algorithm>
 #include <cassert>
+#include <cstdlib>
 
 #include "core.hpp"
 #include "maps.hpp"
@@ -201,13 +202,29 @@ static void build_maps_device(HeffPlan& p, const std::vector<NTerm>& terms, Bloc
     p.T.alloc(tsz);
     cuda_check(cudaMemsetAsync(p.T.p, 0, tsz * 8, st), "memset");     // finite pads
     if (nc > 1) { p.T2.alloc(tsz); cuda_check(cudaMemsetAsync(p.T2.p, 0, tsz * 8, st), "memset"); }
+    // split-K of phase 2: with few output tiles (small / medium bond dimensions) one tile per CTA slot leaves most of the
+    // machine idle in the last wave, so each output block's term range is cut into S parts summed in fixed order
+    int64_t base_tiles = 0;
+    for (int b = 0; b < nblk; ++b)
+        base_tiles += (int64_t)((p.layout[b].rows + GEMM_BM - 1) / GEMM_BM) * ((p.layout[b].cols + GEMM_BN - 1) / GEMM_BN);
+    int S = 1;
+    {
+        int dev = 0, sms = 148;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        const int64_t target = (int64_t)sms * 3 * 6;          // about six tiles per resident CTA slot
+        if (base_tiles > 0) S = (int)std::min<int64_t>(16, std::max<int64_t>(1, (target + base_tiles - 1) / base_tiles));
+        if (const char* g = std::getenv("DMRG_B200_SPLITK")) S = std::max(1, std::min(16, std::atoi(g)));
+    }
+    p.split = S;
+    if (S > 1) p.ypart.alloc((size_t)(S - 1) * (size_t)std::max<int64_t>(p.nnz, 1));
     // ---- pass B: descriptors of every chunk ------------------------------------------------------------------------------------
     p.chunks.resize(nc);
     p.ev_p1.resize(nc); p.ev_p2.resize(nc);
     double ngemm = mb.ngemm;
     for (int c = 0; c < nc; ++c) {
         MapChunkOut o;
-        maps_chunk(cx, cbegin[c], cbegin[c + 1], c == 0, (c & 1) ? p.T2.p : p.T.p, o, dev_alloc, dev_free, st);
+        maps_chunk(cx, cbegin[c], cbegin[c + 1], c == 0, (c & 1) ? p.T2.p : p.T.p, S, p.ypart.p, p.nnz, o, dev_alloc, dev_free, st);
         if ((size_t)o.t_doubles > tsz) throw std::logic_error("heff: intermediate buffer bound violated");
         adopt(p.chunks[c].p1, o.tasks1, o.ntasks1, o.segs1, o.nsegs1, o.tiles1, o.ntiles1, o.flops1);
         adopt(p.chunks[c].p2, o.tasks2, o.ntasks2, o.segs2, o.nsegs2, o.tiles2, o.ntiles2, o.flops2);
@@ -217,6 +234,11 @@ static void build_maps_device(HeffPlan& p, const std::vector<NTerm>& terms, Bloc
         cuda_check(cudaEventCreateWithFlags(&p.ev_p2[c], cudaEventDisableTiming), "event");
     }
     cuda_check(cudaEventCreateWithFlags(&p.ev_in, cudaEventDisableTiming), "event");
+    if (S > 1) {
+        MapChunkOut r;
+        maps_reduce(cx, S, p.ypart.p, p.nnz, r, dev_alloc, dev_free, st);
+        adopt(p.reduce, r.tasks2, r.ntasks2, r.segs2, r.nsegs2, r.tiles2, r.ntiles2, 0.0);
+    }
     p.f_alg = mb.f_alg; p.ngemm = (int64_t)ngemm;
     p.b_alg = mb.b_ops + 16.0 * (double)p.nnz;
     // block tables for the diagonal / padding kernels
@@ -412,7 +434,7 @@ void heff_apply(HeffPlan& p, const double* x_dev, double* y_dev, Engine& eng) {
     // accumulation order into y is fixed (bit-reproducible); T is double buffered (chunk parity).
     const int nc = (int)p.chunks.size();
     if (nc == 1 || eng.trace) {
-        for (auto& c : p.chunks) { run(c.p1, eng); run(c.p2, eng); }
+        for (auto& c : p.chunks) { run(c.p1, eng); run(c.p2, eng); if (p.split > 1) run(p.reduce, eng); }
     } else {
         cuda_check(cudaEventRecord(p.ev_in, eng.stream), "event record");
         cuda_check(cudaStreamWaitEvent(eng.stream2, p.ev_in, 0), "stream wait");
@@ -422,6 +444,7 @@ void heff_apply(HeffPlan& p, const double* x_dev, double* y_dev, Engine& eng) {
             cuda_check(cudaEventRecord(p.ev_p1[c], eng.stream), "event record");
             cuda_check(cudaStreamWaitEvent(eng.stream2, p.ev_p1[c], 0), "stream wait");
             run(p.chunks[c].p2, eng, eng.stream2);
+            if (p.split > 1) run(p.reduce, eng, eng.stream2);
             cuda_check(cudaEventRecord(p.ev_p2[c], eng.stream2), "event record");
         }
         cuda_check(cudaStreamWaitEvent(eng.stream, p.ev_p2[nc - 1], 0), "stream wait");

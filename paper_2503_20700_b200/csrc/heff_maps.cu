@@ -215,8 +215,16 @@ __global__ void k_emit_p1(MapCtx cx, const int64_t* toff, const int* trank, cons
 }
 
 // ---- per chunk: segments of every output block, output-major so that a prefix sum groups them by task -----------------
+// split-K of phase 2: the chunk's term range [0, ntc) is cut into S contiguous parts; part s starts at split_begin
+__device__ __host__ __forceinline__ int split_begin(int s, int ntc, int S) { return (int)(((int64_t)ntc * s) / S); }
+__device__ __forceinline__ int split_part(int rel, int ntc, int S) {
+    int s = (int)(((int64_t)rel * S) / ntc);
+    while (s + 1 < S && split_begin(s + 1, ntc, S) <= rel) ++s;
+    while (s > 0 && split_begin(s, ntc, S) > rel) --s;
+    return s;
+}
 template <bool EMIT>
-__global__ void k_p2(MapCtx cx, int t0, int t1, const int* pos, const int64_t* toff, double* Tbuf, int* cnt, Seg* segs,
+__global__ void k_p2(MapCtx cx, int t0, int t1, int S, const int* pos, const int64_t* toff, double* Tbuf, int* cnt, Seg* segs,
                      double* wK, int* nident, double* flops) {
     const int ntc = t1 - t0;
     const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -255,18 +263,42 @@ __global__ void k_p2(MapCtx cx, int t0, int t1, const int* pos, const int64_t* t
         fl += 2.0 * ob.rows * (double)ob.cols * s.K;
     }
     if (!EMIT) { cnt[idx] = n; return; }
-    if (ksum != 0.0) { atomicAdd(&wK[bo], ksum); atomicAdd(flops, fl); }
-    if (idn) atomicAdd(&nident[bo], idn);
+    const int part = split_part(ti - t0, ntc, S);            // split-K: which part of the chunk's term range
+    if (ksum != 0.0) { atomicAdd(&wK[(size_t)part * cx.nblk + bo], ksum); atomicAdd(flops, fl); }
+    if (idn) atomicAdd(&nident[(size_t)part * cx.nblk + bo], idn);
 }
-__global__ void k_tasks2(MapCtx cx, int ntc, const int* pos, const int* nident, int accum, Task* tasks) {
+// task (part s, block b): part 0 accumulates into y, parts >= 1 write partial sums to ypart (added to y by the
+// reduce launch in part order, so the summation order stays fixed)
+__global__ void k_tasks2(MapCtx cx, int ntc, int S, const int* pos, const int* nident, int accum, double* ypart,
+                         int64_t nnz, Task* tasks) {
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= cx.nblk * S) return;
+    const int s = idx / cx.nblk, b = idx % cx.nblk;
+    const MapBlock& ob = cx.blocks[b];
+    Task t;
+    t.C = s == 0 ? cx.y + ob.off : ypart + (size_t)(s - 1) * nnz + ob.off;
+    t.ldc = ob.cols; t.M = ob.rows; t.N = ob.cols;
+    const int a0 = split_begin(s, ntc, S), a1 = split_begin(s + 1, ntc, S);
+    t.seg_begin = pos[(size_t)b * ntc + a0];
+    t.seg_count = pos[(size_t)b * ntc + a1] - t.seg_begin;       // pos has nblk * ntc + 1 entries: a1 == ntc is the next block's start
+    t.flags = (s == 0 && accum) ? TASK_ACCUM : 0; t.ngemm = t.seg_count - nident[idx];
+    tasks[idx] = t;
+}
+// reduce launch: y block += sum_s ypart[s] block (identity-B segments only), built once per plan
+__global__ void k_reduce(MapCtx cx, int S, const double* ypart, int64_t nnz, Task* tasks, Seg* segs) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= cx.nblk) return;
     const MapBlock& ob = cx.blocks[b];
     Task t;
     t.C = cx.y + ob.off; t.ldc = ob.cols; t.M = ob.rows; t.N = ob.cols;
-    t.seg_begin = pos[(size_t)b * ntc]; t.seg_count = pos[(size_t)(b + 1) * ntc] - t.seg_begin;
-    t.flags = accum ? TASK_ACCUM : 0; t.ngemm = t.seg_count - nident[b];
+    t.seg_begin = b * (S - 1); t.seg_count = S - 1; t.flags = TASK_ACCUM; t.ngemm = 0;
     tasks[b] = t;
+    for (int s = 1; s < S; ++s) {
+        Seg g;
+        g.A = ypart + (size_t)(s - 1) * nnz + ob.off; g.lda = ob.cols; g.B = nullptr; g.ldb = 0; g.K = 0;
+        g.flags = SEG_IDENT_B; g.alpha = 1.0;
+        segs[b * (S - 1) + s - 1] = g;
+    }
 }
 
 // ---- tiles: even split at the 8-row fragment level (same rule as finalize in block.cpp), heaviest first ---------------
@@ -373,8 +405,20 @@ void maps_usage(const MapCtx& cx, std::vector<double>& usage_host, MapBuild& out
     cudaStreamSynchronize(st);
 }
 
-void maps_chunk(const MapCtx& cx, int t0, int t1, bool first_chunk, double* Tbuf, MapChunkOut& out, MapAlloc alloc,
-                void (*dealloc)(void*), cudaStream_t st) {
+void maps_reduce(const MapCtx& cx, int S, double* ypart, int64_t nnz, MapChunkOut& out, MapAlloc alloc,
+                 void (*dealloc)(void*), cudaStream_t st) {
+    Scratch sc(alloc, dealloc);
+    out.ntasks2 = cx.nblk; out.nsegs2 = cx.nblk * (S - 1);
+    out.tasks2 = (Task*)alloc(std::max<size_t>(cx.nblk, 1) * sizeof(Task));
+    out.segs2 = (Seg*)alloc(std::max<size_t>(out.nsegs2, 1) * sizeof(Seg));
+    k_reduce<<<nblocks(cx.nblk, 128), 128, 0, st>>>(cx, S, ypart, nnz, out.tasks2, out.segs2);
+    double* w0 = sc.get<double>((size_t)cx.nblk, st, true);
+    out.ntiles2 = build_tiles(out.tasks2, cx.nblk, w0, &out.tiles2, sc, alloc, st);
+    cudaStreamSynchronize(st);
+}
+
+void maps_chunk(const MapCtx& cx, int t0, int t1, bool first_chunk, double* Tbuf, int S, double* ypart, int64_t nnz,
+                MapChunkOut& out, MapAlloc alloc, void (*dealloc)(void*), cudaStream_t st) {
     Scratch sc(alloc, dealloc);
     auto pol = thrust::cuda::par.on(st);
     const int ntc = t1 - t0;
@@ -405,20 +449,21 @@ void maps_chunk(const MapCtx& cx, int t0, int t1, bool first_chunk, double* Tbuf
     // ---- phase 2: one task per psi block, segments in (block, term) order ------------------------------------------------------
     const int64_t npair = (int64_t)cx.nblk * ntc;
     int* pos = sc.get<int>((size_t)npair + 1, st, true);
-    if (npair > 0) k_p2<false><<<nblocks(npair, 128), 128, 0, st>>>(cx, t0, t1, nullptr, toff, Tbuf, pos, nullptr, nullptr, nullptr, nullptr);
+    if (npair > 0) k_p2<false><<<nblocks(npair, 128), 128, 0, st>>>(cx, t0, t1, S, nullptr, toff, Tbuf, pos, nullptr, nullptr, nullptr, nullptr);
     thrust::exclusive_scan(pol, pos, pos + npair + 1, pos);
     int nsegs2 = 0;
     cudaMemcpyAsync(&nsegs2, pos + npair, 4, cudaMemcpyDeviceToHost, st);
     cudaStreamSynchronize(st);
     out.nsegs2 = nsegs2;
-    out.ntasks2 = cx.nblk;
-    out.tasks2 = (Task*)alloc(std::max<size_t>(cx.nblk, 1) * sizeof(Task));
+    out.ntasks2 = cx.nblk * S;
+    out.tasks2 = (Task*)alloc(std::max<size_t>((size_t)cx.nblk * S, 1) * sizeof(Task));
     out.segs2 = (Seg*)alloc(std::max<size_t>(nsegs2, 1) * sizeof(Seg));
-    double* wK2 = sc.get<double>((size_t)cx.nblk, st, true);
-    int* nident = sc.get<int>((size_t)cx.nblk, st, true);
-    if (npair > 0) k_p2<true><<<nblocks(npair, 128), 128, 0, st>>>(cx, t0, t1, pos, toff, Tbuf, nullptr, out.segs2, wK2, nident, fl + 1);
-    k_tasks2<<<nblocks(cx.nblk, 256), 256, 0, st>>>(cx, ntc, pos, nident, first_chunk ? 0 : 1, out.tasks2);
-    out.ntiles2 = build_tiles(out.tasks2, cx.nblk, wK2, &out.tiles2, sc, alloc, st);
+    double* wK2 = sc.get<double>((size_t)cx.nblk * S, st, true);
+    int* nident = sc.get<int>((size_t)cx.nblk * S, st, true);
+    if (npair > 0) k_p2<true><<<nblocks(npair, 128), 128, 0, st>>>(cx, t0, t1, S, pos, toff, Tbuf, nullptr, out.segs2, wK2, nident, fl + 1);
+    k_tasks2<<<nblocks((int64_t)cx.nblk * S, 256), 256, 0, st>>>(cx, ntc, S, pos, nident, first_chunk ? 0 : 1, ypart, nnz, out.tasks2);
+    out.ntiles2 = build_tiles(out.tasks2, cx.nblk * S, wK2, &out.tiles2, sc, alloc, st);
+    out.split = S;
     double hf[2] = {0, 0};
     cudaMemcpyAsync(hf, fl, sizeof hf, cudaMemcpyDeviceToHost, st);
     cudaStreamSynchronize(st);

@@ -35,6 +35,7 @@ struct MapChunkOut {                                  // device-resident launch 
     Task* tasks2 = nullptr; Seg* segs2 = nullptr; Tile* tiles2 = nullptr; int ntasks2 = 0, nsegs2 = 0, ntiles2 = 0;
     double flops1 = 0, flops2 = 0;
     int64_t t_doubles = 0;                            // intermediate buffer the chunk needs
+    int split = 1;                                    // split-K parts of phase 2 actually used
 };
 
 // Scratch + results of the builder.  All device allocations go through alloc / are owned by the caller afterwards.
@@ -51,7 +52,11 @@ struct MapBuild {
 typedef void* (*MapAlloc)(size_t bytes);
 void maps_usage(const MapCtx& cx, std::vector<double>& usage_host, MapBuild& out, MapAlloc alloc, void (*dealloc)(void*),
                 cudaStream_t st);
-void maps_chunk(const MapCtx& cx, int t0, int t1, bool first_chunk, double* Tbuf, MapChunkOut& out, MapAlloc alloc,
-                void (*dealloc)(void*), cudaStream_t st);
+// S: split-K parts of phase 2 (part 0 -> y, parts s >= 1 -> ypart + (s-1) * nnz); maps_reduce builds the launch that adds
+// the partial sums into y (tasks2 / segs2 / tiles2 of `out`).
+void maps_chunk(const MapCtx& cx, int t0, int t1, bool first_chunk, double* Tbuf, int S, double* ypart, int64_t nnz,
+                MapChunkOut& out, MapAlloc alloc, void (*dealloc)(void*), cudaStream_t st);
+void maps_reduce(const MapCtx& cx, int S, double* ypart, int64_t nnz, MapChunkOut& out, MapAlloc alloc,
+                 void (*dealloc)(void*), cudaStream_t st);
 
 }  // namespace dmrg
