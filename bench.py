@@ -44,7 +44,7 @@ def parse_args():
     ap.add_argument("--config", type=int, default=4, help="BASELINE config 1..5 (default 4: the metric's workload)")
     ap.add_argument("--D", type=int, default=0, help="bond dimension override (0 = the config's)")
     ap.add_argument("--bond", type=int, default=-1, help="two-site bond (default mid-chain k/2-1)")
-    ap.add_argument("--extras", type=int, default=1, help="1: also time sweeps + RDM on config 1; 2: on configs 1-3")
+    ap.add_argument("--extras", type=int, default=2, help="1: also time sweeps + RDM on config 1; 2: on configs 1-3")
     ap.add_argument("--cpu-baseline", type=int, default=1)
     ap.add_argument("--sample-config", type=int, default=2, help="config of the oracle's bounded sample")
     ap.add_argument("--sample-D", type=int, default=96)

@@ -255,6 +255,24 @@ namespace dmrg {
 
 namespace {
 
+// Bump allocator over one device allocation made per dmrg_rdm12 call: the pass needs thousands of short-lived
+// intermediates per centre, and a cudaMalloc / cudaFree pair each (the free synchronises the device) dominated its time.
+struct Arena {
+    DevVec<double> buf;
+    size_t used = 0;
+    std::vector<DevVec<double>> overflow;         // requests that do not fit fall back to their own allocation
+    void init(size_t doubles) { buf.alloc(doubles); used = 0; }
+    void reset() { used = 0; overflow.clear(); }
+    double* get(size_t n) {
+        n = (n + 1) & ~(size_t)1;                 // keep 16-byte alignment
+        if (used + n <= buf.n) { double* p = buf.p + used; used += n; return p; }
+        overflow.emplace_back();
+        overflow.back().alloc(n);
+        return overflow.back().p;
+    }
+};
+Arena g_arena;
+
 // E[stack][row * ncol + col] for every stack referenced by the records of each group
 struct GroupResult { std::map<int, std::vector<double>> E; int ncol = 0; };
 
@@ -268,17 +286,17 @@ void evaluate_group(CentreCtx& cx, ColGroup& g, const std::vector<int>& stacks, 
     for (int s : stacks) out.E[s].assign((size_t)L.stacks[s].members.size() * ncol, 0.0);
     if (cls.nnz == 0 || ncol == 0) return;
     const int64_t ld = cls.ld;
-    const int64_t cap = eng.t_capacity();
+    const int64_t cap = (int64_t)g_arena.buf.n;
     int chunk_cols = (int)std::max<int64_t>(1, std::min<int64_t>(ncol, (cap / 2) / ld));
     for (int c0 = 0; c0 < ncol; c0 += chunk_cols) {
         const int nc = std::min(chunk_cols, ncol - c0);
-        DevVec<double> Mbuf;
-        Mbuf.alloc((size_t)nc * ld);
+        g_arena.reset();
+        struct { double* p; } Mbuf;
+        Mbuf.p = g_arena.get((size_t)nc * ld);
         cuda_check(cudaMemsetAsync(Mbuf.p, 0, (size_t)nc * ld * 8, eng.stream), "memset");
         // ---- phase 1: T[(Y, l, si)] = psi[(l,si)] Y^T ; phase 2: M blocks ------------------------------------------------
         GemmBatch p1, p2;
         std::unordered_map<uint64_t, std::pair<double*, int>> tcache;       // (yid, l, si) -> (T, ld)
-        std::vector<DevVec<double>> tbufs;
         for (int cc = 0; cc < nc; ++cc) {
             const uint32_t key = g.keys[c0 + cc];
             const int yid = (int)(key >> 8);
@@ -304,11 +322,10 @@ void evaluate_group(CentreCtx& cx, ColGroup& g, const std::vector<int>& stacks, 
                     auto it = tcache.find(tk);
                     if (it == tcache.end()) {
                         const int dro = R.basis[v.out].d;
-                        tbufs.emplace_back();
-                        tbufs.back().alloc((size_t)kb->rows * pad2(dro));
-                        const int t1 = p1.add_task(tbufs.back().p, pad2(dro), kb->rows, dro, 0);
+                        double* tp = g_arena.get((size_t)kb->rows * pad2(dro));
+                        const int t1 = p1.add_task(tp, pad2(dro), kb->rows, dro, 0);
                         p1.add_seg(t1, kb->ptr, kb->ld, v.ptr, v.ld, kb->cols, v.trans ? 0 : SEG_TRANS_B, 1.0);
-                        it = tcache.emplace(tk, std::make_pair(tbufs.back().p, pad2(dro))).first;
+                        it = tcache.emplace(tk, std::make_pair(tp, pad2(dro))).first;
                     }
                     tptr = it->second.first; tld = it->second.second;
                 } else if (kb->r != bb->r) continue;
@@ -332,14 +349,16 @@ void evaluate_group(CentreCtx& cx, ColGroup& g, const std::vector<int>& stacks, 
             int64_t kc = (ld + nsplit - 1) / nsplit;
             kc = (kc + 15) & ~(int64_t)15;
             nsplit = (int)((ld + kc - 1) / kc);
-            DevVec<double> part, Ed;
-            Ed.alloc((size_t)nrows * nc);
+            struct { double* p; } part, Ed;
+            part.p = nullptr;
+            const size_t arena_mark = g_arena.used;
+            Ed.p = g_arena.get((size_t)nrows * nc);
             GemmBatch gb, red;
             if (nsplit == 1) {
                 const int t = gb.add_task(Ed.p, nc, nrows, nc, 0);
                 gb.add_seg(t, stk.base, (int)ld, Mbuf.p, (int)ld, (int)ld, SEG_TRANS_B, 1.0);
             } else {
-                part.alloc((size_t)nsplit * nrows * nc);
+                part.p = g_arena.get((size_t)nsplit * nrows * nc);
                 const int tr = red.add_task(Ed.p, nc, nrows, nc, 0);
                 for (int p = 0; p < nsplit; ++p) {
                     const int64_t k0 = (int64_t)p * kc, kk = std::min<int64_t>(kc, ld - k0);
@@ -357,6 +376,7 @@ void evaluate_group(CentreCtx& cx, ColGroup& g, const std::vector<int>& stacks, 
             cuda_check(cudaMemcpy2DAsync(E.data() + c0, (size_t)ncol * 8, Ed.p, (size_t)nc * 8, (size_t)nc * 8, nrows,
                                          cudaMemcpyDeviceToHost, eng.stream), "E download");
             cuda_check(cudaStreamSynchronize(eng.stream), "E download");
+            g_arena.used = arena_mark;                         // Ed / part of this stack are dead
         }
     }
 }
@@ -376,6 +396,8 @@ void rdm12(Engine& eng, double* gamma, double* Gamma) {
         if (mps.sites[p].gauge != 'R')
             throw Error(-2, "rdm12: the MPS must be right-canonical with its centre on site 0 (as imported or as left by dmrg_sweep)");
     eng.rdm_bytes = 0; eng.rdm_flops = 0; eng.rdm_stream_ms = 0;
+    g_arena.init((size_t)std::min<int64_t>(eng.t_capacity(), (int64_t)1 << 29));   // at most 4 GiB of intermediates at a time
+    struct ArenaRelease { ~ArenaRelease() { g_arena.overflow.clear(); g_arena.buf.release(); } } arena_release;
     std::memset(gamma, 0, sizeof(double) * (size_t)k * k);
     if (want2) std::memset(Gamma, 0, sizeof(double) * (size_t)k * k * k * k);
     // right blocks with the one-index operators of the sites > c

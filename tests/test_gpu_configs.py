@@ -111,3 +111,48 @@ def test_config4_D4096_full_size_properties(lib):
         assert 0 < st["f_exec"] <= st["f_alg"] and st["nterms"] > 6000
     finally:
         lib.dmrg_destroy(ctx)
+
+
+def test_config5_D1024_properties(lib):
+    """configs[4] (82-site PAH-like chain of fused hexagons, CAS(82,82)) at a reduced bond dimension: the oracle cannot
+    reach it in bounded time (reading S27), so the check is by properties that hold at any size - symmetry,
+    linearity, bit-reproducibility, <e_j|H|e_j> = diag_j - on the device-built block maps of a 13 000-term bond."""
+    import torch
+    cfg = make_config(5)
+    k, n, D = cfg["k"], cfg["n_elec"], 1024
+    i = k // 2 - 1
+    mps = random_mps(k, n, 0, D, seed=cfg["seed"] + 1000, gauge="LR:%d" % i)
+    ctx = lib.dmrg_create(k, n, 0, cfg["h"], cfg["eri"], keep_env_stack=0)
+    try:
+        lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, 0)
+        lib.dmrg_prepare_bond(ctx, i)
+        nnz, lay = lib.dmrg_heff_layout(ctx, i)
+        assert nnz == sum(b[4] * b[5] for b in lay)
+        g = torch.Generator(device="cpu").manual_seed(11)
+        x = torch.randn(nnz, dtype=torch.float64, generator=g).cuda()
+        p = torch.randn(nnz, dtype=torch.float64, generator=g).cuda()
+        x /= x.norm()
+        p /= p.norm()
+        y, q, z, y2 = (torch.empty_like(x) for _ in range(4))
+        lib.dmrg_heff_apply(ctx, i, x, y)
+        lib.dmrg_heff_apply(ctx, i, p, q)
+        lib.dmrg_heff_apply(ctx, i, 0.5 * x - 2.0 * p, z)
+        lib.dmrg_heff_apply(ctx, i, x, y2)
+        torch.cuda.synchronize()
+        assert torch.isfinite(y).all() and float(y.norm()) > 0
+        assert torch.equal(y, y2)
+        assert abs(float(p @ y) - float(q @ x)) <= 1e-11 * float(y.norm())
+        assert float((z - (0.5 * y - 2.0 * q)).norm()) <= 1e-12 * float(z.norm())
+        d = torch.empty_like(x)
+        lib.dmrg_heff_diag(ctx, i, d)
+        torch.cuda.synchronize()
+        for j in (1, nnz // 2, nnz - 2):
+            e = torch.zeros_like(x)
+            e[j] = 1.0
+            lib.dmrg_heff_apply(ctx, i, e, z)
+            torch.cuda.synchronize()
+            assert abs(float(z[j]) - float(d[j])) <= 1e-11 * max(1.0, abs(float(d[j])))
+        st = lib.dmrg_heff_stats(ctx, i)
+        assert 0 < st["f_exec"] <= st["f_alg"] and st["nterms"] > 13000
+    finally:
+        lib.dmrg_destroy(ctx)
