@@ -44,7 +44,7 @@ def parse_args():
     ap.add_argument("--config", type=int, default=4, help="BASELINE config 1..5 (default 4: the metric's workload)")
     ap.add_argument("--D", type=int, default=0, help="bond dimension override (0 = the config's)")
     ap.add_argument("--bond", type=int, default=-1, help="two-site bond (default mid-chain k/2-1)")
-    ap.add_argument("--extras", type=int, default=2, help="1: also time sweeps + RDM on config 1; 2: on configs 1-3")
+    ap.add_argument("--extras", type=int, default=2, help="1: also time sweeps + RDM on config 1; 2: on configs 1-3; 3: + one sweep of config 4 at D=1024")
     ap.add_argument("--cpu-baseline", type=int, default=1)
     ap.add_argument("--sample-config", type=int, default=2, help="config of the oracle's bounded sample")
     ap.add_argument("--sample-D", type=int, default=96)
@@ -221,9 +221,10 @@ def time_small_extras(P, torch, peaks, level):
     1-3 with one sweep each (from a seeded random MPS, so bond dimensions are saturated from the start)."""
     from synth import make_config, random_mps, mps_to_blob_arrays
     out = {}
-    for cid, nsweep in ((1, 3), (2, 1), (3, 1))[: (1 if level == 1 else 3)]:
+    plan = [(1, 3, 0), (2, 1, 0), (3, 1, 0), (4, 1, 1024)]     # (config, sweeps, D override); config 4 at D = 1024: the
+    for cid, nsweep, Dov in plan[: {1: 1, 2: 3}.get(level, 4)]:  # environment stack of D = 4096 does not fit one GPU yet
         cfg = make_config(cid)
-        k, n, D = cfg["k"], cfg["n_elec"], cfg["D"]
+        k, n, D = cfg["k"], cfg["n_elec"], Dov or cfg["D"]
         mps = random_mps(k, n, 0, D, seed=cfg["seed"] + 1000, gauge="R")
         ctx = P.dmrg_create(k, n, 0, cfg["h"], cfg["eri"])
         rec = {"workload": "%s D=%d" % (cfg["name"], D)}
@@ -241,6 +242,10 @@ def time_small_extras(P, torch, peaks, level):
                             "matvec_seconds_last_sweep": tmv, "matvec_f_alg_last_sweep": fl,
                             "matvec_tflops_last_sweep": fl / tmv / 1e12 if tmv > 0 else None,
                             "max_kept": int(max(b["kept"] for b in r["bonds"]))}
+            if cid > 3:
+                rec["rdm12"] = {"skipped": "the round-1 RDM pass keeps all two-index operators of one side (DESIGN.md 5.4)"}
+                out["config%d" % cid] = rec
+                continue
             try:
                 t0 = time.perf_counter()
                 g, G = P.dmrg_rdm12(ctx, k, True)
@@ -283,9 +288,11 @@ def run_ours(args):
                         workspace_bytes=int(args.workspace_gb * (1 << 30)))
     P.dmrg_mps_import(ctx, blob, k, n, 0)
     t_env = time.perf_counter()
+    f_env = P.dmrg_flops_total(ctx)
     P.dmrg_prepare_bond(ctx, i)                      # renormalisation of both environments + block maps (a1, a5)
     torch.cuda.synchronize()
     t_env = time.perf_counter() - t_env
+    f_env = P.dmrg_flops_total(ctx) - f_env          # executed flops of all blocking steps (row a5)
     nnz, layout = P.dmrg_heff_layout(ctx, i)
     st = P.dmrg_heff_stats(ctx, i)
     g = torch.Generator(device="cpu").manual_seed(1234 + rank)
@@ -364,7 +371,8 @@ def run_ours(args):
                                    "replicas only for N>1" % (cfg["name"], D, i),
                        "nnz_psi": nnz, "psi_blocks": len(layout), "terms": st["nterms"], "gemms": st["ngemm"],
                        "l2": "inputs larger than L2 (operator blocks %.1f GB)" % ((st["b_alg"] - 16.0 * nnz) / 1e9),
-                       "device_gb": dev_bytes / 1e9, "env_build_s": t_env, "setup_s": t_setup},
+                       "device_gb": dev_bytes / 1e9, "env_build_s": t_env, "env_build_flops": f_env,
+                       "env_build_tflops_wallclock": f_env / t_env / 1e12, "setup_s": t_setup},
             "ms_per_step_minmax": [min(per_step), max(per_step)],
             "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": 8 * nnz, "d2h_bytes_per_step": 8 * nnz,
                     "ms_per_step": e2e_s * 1e3},

@@ -144,6 +144,9 @@ int dmrg_rdm_stats(dmrg_ctx* ctx, double* seconds, double* bytes_streamed, doubl
 
 /* Number of kernels this library launched on the context since creation (bench.py's gpu_launches). */
 int64_t dmrg_launch_count(const dmrg_ctx* ctx);
+/* Unpadded flops (sum of 2 M N K) of every grouped-GEMM launch of the context since creation: H_eff psi, operator
+ * renormalisation, RDM contractions.  Differences around a call give that call's executed flops. */
+double dmrg_flops_total(const dmrg_ctx* ctx);
 /* Device bytes currently held by the context's arenas. */
 int64_t dmrg_device_bytes(const dmrg_ctx* ctx);
 

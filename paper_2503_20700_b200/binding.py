@@ -55,7 +55,7 @@ class dmrg_sweep_result(C.Structure):
 
 EXPORTS = ["dmrg_default_options", "dmrg_create", "dmrg_destroy", "dmrg_last_error", "dmrg_mps_import",
            "dmrg_mps_export", "dmrg_prepare_bond", "dmrg_heff_layout", "dmrg_heff_apply", "dmrg_heff_diag",
-           "dmrg_heff_stats", "dmrg_sweep", "dmrg_rdm12", "dmrg_rdm_stats", "dmrg_launch_count", "dmrg_device_bytes",
+           "dmrg_heff_stats", "dmrg_sweep", "dmrg_rdm12", "dmrg_rdm_stats", "dmrg_launch_count", "dmrg_flops_total", "dmrg_device_bytes",
            "dmrg_grouped_gemm", "dmrg_last_gemm_ms", "dmrg_fp64_probe"]
 
 lib.dmrg_last_error.restype = C.c_char_p
@@ -64,6 +64,8 @@ lib.dmrg_launch_count.restype = C.c_int64
 lib.dmrg_launch_count.argtypes = [C.c_void_p]
 lib.dmrg_last_gemm_ms.restype = C.c_double
 lib.dmrg_last_gemm_ms.argtypes = []
+lib.dmrg_flops_total.restype = C.c_double
+lib.dmrg_flops_total.argtypes = [C.c_void_p]
 lib.dmrg_device_bytes.restype = C.c_int64
 lib.dmrg_device_bytes.argtypes = [C.c_void_p]
 
@@ -244,3 +246,8 @@ def dmrg_fp64_probe(kind, iters=20000, ctas_per_sm=3, size=8192, reps=3, stream=
 def dmrg_last_gemm_ms():
     """Device milliseconds of the kernel launched by the most recent dmrg_grouped_gemm call."""
     return float(lib.dmrg_last_gemm_ms())
+
+
+def dmrg_flops_total(ctx):
+    """Unpadded flops of every grouped-GEMM launch of the context since creation."""
+    return float(lib.dmrg_flops_total(ctx))

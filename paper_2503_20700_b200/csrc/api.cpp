@@ -141,6 +141,7 @@ int dmrg_destroy(dmrg_ctx* ctx) {
 
 const char* dmrg_last_error(const dmrg_ctx* ctx) { return ctx ? ctx->eng.last_error.c_str() : "null context"; }
 int64_t dmrg_launch_count(const dmrg_ctx* ctx) { return ctx ? ctx->eng.launches : 0; }
+double dmrg_flops_total(const dmrg_ctx* ctx) { return ctx ? ctx->eng.flops_total : 0.0; }
 int64_t dmrg_device_bytes(const dmrg_ctx*) { return g_device_bytes; }
 
 int dmrg_mps_import(dmrg_ctx* ctx, const dmrg_mps_blob* b) {

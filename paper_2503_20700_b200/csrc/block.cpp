@@ -183,6 +183,7 @@ void run(const GemmLaunch& l, Engine& eng, cudaStream_t st) {
     else
         launch_seg_gemm(l.tasks.p, l.segs.p, l.tiles.p, l.ntiles, st);
     eng.launches++;
+    eng.flops_total += l.flops;
     if (eng.trace) {
         cudaEventRecord(e1, st);
         cudaEventSynchronize(e1);

@@ -217,6 +217,7 @@ struct Engine {
     std::map<int, std::unique_ptr<Block>> L, R;   // by bond
     std::unique_ptr<HeffPlan> plan;
     int64_t launches = 0;
+    double flops_total = 0;                       // unpadded flops of every grouped-GEMM launch since creation
     std::string last_error;
     SvdWork* svd = nullptr;
     double rdm_seconds = 0, rdm_bytes = 0, rdm_flops = 0;
