@@ -62,3 +62,37 @@ def test_grouped_gemm_many_segments_spanning_tiles(lib):
     rng = np.random.default_rng(11)
     shapes = [(150, 170, [int(k) for k in rng.integers(1, 90, size=40)]), (257, 129, [300, 7, 64])]
     _case(lib, rng, shapes, False)
+
+
+def test_probe_and_counters(lib):
+    """dmrg_fp64_probe returns plausible ceilings (DMMA within 50-110 % of the nominal 37.2 TFLOP/s of a B200),
+    dmrg_last_gemm_ms times the kernel of the last dmrg_grouped_gemm call, dmrg_flops_total counts unpadded flops."""
+    import torch
+    r = lib.dmrg_fp64_probe(0, iters=4000, ctas_per_sm=3, reps=2)
+    assert 0.5 * 37.2 <= r["tflops"] <= 1.1 * 37.2 and r["ms"] > 0
+    r1 = lib.dmrg_fp64_probe(1, iters=4000, ctas_per_sm=3, reps=2)
+    assert 5.0 <= r1["tflops"] <= 1.1 * 37.2
+    with pytest.raises(lib.binding.DmrgError):
+        lib.dmrg_fp64_probe(7)
+    rng = np.random.default_rng(3)
+    _case(lib, rng, [(128, 96, [64, 32])], False)
+    assert lib.dmrg_last_gemm_ms() > 0.0
+    from synth import random_dense, random_mps, mps_to_blob_arrays
+    k, n = 6, 6
+    h, eri = random_dense(k, 1)
+    ctx = lib.dmrg_create(k, n, 0, h, eri)
+    try:
+        assert lib.dmrg_flops_total(ctx) == 0.0
+        lib.dmrg_mps_import(ctx, mps_to_blob_arrays(random_mps(k, n, 0, 12, seed=2, gauge="LR:2")), k, n, 0)
+        lib.dmrg_prepare_bond(ctx, 2)
+        f0 = lib.dmrg_flops_total(ctx)
+        assert f0 > 0.0
+        nnz, _ = lib.dmrg_heff_layout(ctx, 2)
+        x = np.ones(nnz)
+        y = np.zeros(nnz)
+        lib.dmrg_heff_apply(ctx, 2, x, y)
+        st = lib.dmrg_heff_stats(ctx, 2)
+        assert lib.dmrg_flops_total(ctx) - f0 == st["f_exec"]
+    finally:
+        lib.dmrg_destroy(ctx)
+    torch.cuda.synchronize()
