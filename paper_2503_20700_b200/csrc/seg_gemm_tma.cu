@@ -174,7 +174,8 @@ seg_gemm_tma_kernel(const Task* __restrict__ tasks, const Seg* __restrict__ segs
         // Descriptor pipeline: the dependent chain  tile counter -> Tile -> Task -> first Seg  is spread over four
         // tiles (each load is issued one tile before its result is needed), and inside a tile the next Seg is loaded
         // while the current one is being streamed, so the producer never waits on descriptor latency in steady state.
-        uint32_t pstep = 0;
+        int pstage = 0;
+        uint32_t pphase = 0;                                  // ring position and the parity of its round
         int tslot = 0;
         auto take = [&]() { int v = 0; if (lane == 0) v = atomicAdd(counter, 1); return v; };   // valid on lane 0
         Tile tl_d, tl_c, tl_b;
@@ -213,23 +214,37 @@ seg_gemm_tma_kernel(const Task* __restrict__ tasks, const Seg* __restrict__ segs
             if (lastseg >= 1) nxt = sg[1];
             double ratio = 1.0;                               // != 1 on the first stage of a segment whose alpha differs
             bool rescale = false;
+            // per-segment, per-lane copy state: source pointers of this lane's piece of the A / B panel of the next
+            // stage and their per-stage advance, so that a stage costs pointer increments instead of index arithmetic
+            const int c2 = (lane % LCPR) * 2, r0 = lane / LCPR;   // LDGSTS: this lane's 16-byte column chunk and first row
+            const double* pa = nullptr;
+            const double* pb = nullptr;
+            size_t adv_a = 0, adv_b = 0, row_a = 0, row_b = 0;
+            const uint32_t bytesA = (uint32_t)pad2d(mv) * 8u, bytesB = (uint32_t)pad2d(nv) * 8u;   // bulk row pieces
+            auto seg_setup = [&]() {
+                const size_t lda = (size_t)(uint32_t)cur.lda, ldb = (size_t)(uint32_t)cur.ldb;
+                if (cur.flags & SEG_TRANS_A) { pa = cur.A + (uint32_t)m0 + (uint32_t)lane * lda; adv_a = BK * lda; }
+                else { pa = cur.A + (uint32_t)(m0 + r0) * lda + (uint32_t)c2; adv_a = BK; row_a = LRS * lda; }
+                if (cur.flags & SEG_TRANS_B) { pb = cur.B + (uint32_t)(n0 + r0) * ldb + (uint32_t)c2; adv_b = BK; row_b = LRS * ldb; }
+                else { pb = cur.B + (uint32_t)n0 + (uint32_t)lane * ldb; adv_b = BK * ldb; }
+            };
+            if (!stop && lastseg >= 0) seg_setup();
             do {                                              // one pipeline stage per iteration
-                const int stage = pstep % ST2;
-                mbar_wait(&empty_bar[stage], ((pstep / ST2) & 1) ^ 1);
-                double* As = smem + stage * STAGE_DOUBLES;
+                mbar_wait(&empty_bar[pstage], pphase ^ 1);
+                double* As = smem + pstage * STAGE_DOUBLES;
                 double* Bs = As + PANEL;
                 const bool compute = !stop && s <= lastseg;
-                int kv = 0, rowsA = 0, rowsB = 0;
-                uint32_t bytesA = 0, bytesB = 0;
+                int kv = 0;
+                uint32_t tx = 0;
                 bool last = true;
                 if (compute) {
                     kv = min(BK, cur.K - lk);
-                    if (cur.flags & SEG_TRANS_A) { rowsA = kv; bytesA = (uint32_t)pad2d(mv) * 8u; }    // bulk rows [k][m]
-                    if (!(cur.flags & SEG_TRANS_B)) { rowsB = kv; bytesB = (uint32_t)pad2d(nv) * 8u; } // bulk rows [k][n]
+                    if (cur.flags & SEG_TRANS_A) tx += (uint32_t)kv * bytesA;      // bulk rows [k][m]
+                    if (!(cur.flags & SEG_TRANS_B)) tx += (uint32_t)kv * bytesB;   // bulk rows [k][n]
                     last = (s == lastseg) && (lk + BK >= cur.K);
                 }
                 if (lane == 0) {
-                    StageInfo& in = info[stage];
+                    StageInfo& in = info[pstage];
                     in.alpha = compute ? cur.alpha : 0.0;
                     in.ratio = ratio;
                     in.kv = kv;
@@ -242,33 +257,29 @@ seg_gemm_tma_kernel(const Task* __restrict__ tasks, const Seg* __restrict__ segs
                         ti.ldc = tk.ldc; ti.mv = mv; ti.nv = nv; ti.m0 = m0; ti.n0 = n0; ti.tflags = tk.flags;
                         in.tslot = tslot;
                     }
-                    mbar_arrive_expect_tx(&full_bar[stage], (uint32_t)rowsA * bytesA + (uint32_t)rowsB * bytesB);
+                    mbar_arrive_expect_tx(&full_bar[pstage], tx);
                 }
                 __syncwarp();
                 if (compute) {
-                    const int c2 = (lane % LCPR) * 2, r0 = lane / LCPR;        // LDGSTS: this lane's 16-byte column chunk and first row
                     if (cur.flags & SEG_TRANS_A) {
-                        const double* src = cur.A + (size_t)lk * cur.lda + m0;
-                        for (int r = lane; r < rowsA; r += 32) bulk_g2s(As + r * LDM, src + (size_t)r * cur.lda, bytesA, &full_bar[stage]);
+                        if (lane < kv) bulk_g2s(As + lane * LDM, pa, bytesA, &full_bar[pstage]);   // BK <= 32: one row per lane
                     } else if (c2 < kv) {
-                        const double* src = cur.A + (size_t)(m0 + r0) * cur.lda + lk + c2;
+                        const double* src = pa;
                         double* dst = As + r0 * LDK + c2;
-                        const size_t step = (size_t)LRS * cur.lda;
 #pragma unroll 4
-                        for (int r = r0; r < mv; r += LRS) { ldgsts16(dst, src); dst += LRS * LDK; src += step; }
+                        for (int r = r0; r < mv; r += LRS) { ldgsts16(dst, src); dst += LRS * LDK; src += row_a; }
                     }
                     if (cur.flags & SEG_TRANS_B) {
                         if (c2 < kv) {
-                            const double* src = cur.B + (size_t)(n0 + r0) * cur.ldb + lk + c2;
+                            const double* src = pb;
                             double* dst = Bs + r0 * LDK + c2;
-                            const size_t step = (size_t)LRS * cur.ldb;
 #pragma unroll 4
-                            for (int r = r0; r < nv; r += LRS) { ldgsts16(dst, src); dst += LRS * LDK; src += step; }
+                            for (int r = r0; r < nv; r += LRS) { ldgsts16(dst, src); dst += LRS * LDK; src += row_b; }
                         }
                     } else {
-                        const double* src = cur.B + (size_t)lk * cur.ldb + n0;
-                        for (int r = lane; r < rowsB; r += 32) bulk_g2s(Bs + r * LDM, src + (size_t)r * cur.ldb, bytesB, &full_bar[stage]);
+                        if (lane < kv) bulk_g2s(Bs + lane * LDM, pb, bytesB, &full_bar[pstage]);
                     }
+                    pa += adv_a; pb += adv_b;
                     lk += BK;
                     if (lk >= cur.K) {                                // next segment: already in registers
                         lk = 0;
@@ -276,14 +287,15 @@ seg_gemm_tma_kernel(const Task* __restrict__ tasks, const Seg* __restrict__ segs
                         rescale = (s <= lastseg) && (nxt.alpha != cur.alpha);
                         if (rescale) ratio = cur.alpha / nxt.alpha;   // segments with alpha == 0 are dropped by the host
                         cur = nxt;
+                        if (s <= lastseg) seg_setup();
                         if (s + 1 <= lastseg) nxt = sg[s + 1];
                     } else {
                         rescale = false;
                     }
                 }
-                ldgsts_arrive_noinc(&full_bar[stage]);                // fires when this lane's LDGSTS of the stage have landed
+                ldgsts_arrive_noinc(&full_bar[pstage]);               // fires when this lane's LDGSTS of the stage have landed
                 first = false;
-                ++pstep;
+                if (++pstage == ST2) { pstage = 0; pphase ^= 1; }
             } while (!stop && s <= lastseg);
             if (stop) break;
         }
