@@ -32,7 +32,7 @@ N_SM = 148
 BF16_NOMINAL_TF = 2250.0
 # dram__bytes_read.sum + dram__bytes_write.sum over the 56 seg_gemm_tma_kernel launches of one H_eff psi at config 4,
 # D = 4096, bond 26, from the ncu capture profiles/r01_step_dram_heff_cfg4.md (same launch configuration as this bench)
-NCU_TRAFFIC_BYTES_PER_STEP_CFG4 = 3.7423e12
+NCU_TRAFFIC_BYTES_PER_STEP_CFG4 = 3.31e12
 
 
 def parse_args():
