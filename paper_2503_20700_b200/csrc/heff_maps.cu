@@ -329,13 +329,7 @@ __global__ void k_tile_emit(const Task* tasks, int ntasks, const int* pos, const
             const int mv = min(pm, M - m0), nv = min(pn, N - n0);
             Tile tl; tl.task = t; tl.m0 = m0; tl.n0 = n0; tl.mv = mv; tl.nv = nv;
             tiles[w] = tl;
-#ifdef MAPS_TILE_WEIGHT
-            weight[w] = (wK[t] + 16.0) * ((mv + 7) / 8) * ((nv + 7) / 8);
-#else
-            // all tiles of one task share one sort key (the task's cost), so they stay adjacent in the tile list: CTAs
-            // that pick them up together walk the same K range together and share its operand panels through L2
-            weight[w] = (wK[t] + 16.0) * ((M + 7) / 8) * ((N + 7) / 8);
-#endif
+            weight[w] = (wK[t] + 16.0) * ((mv + 7) / 8) * ((nv + 7) / 8);   // (a per-task key was tried: no gain)
             ++w;
         }
 }
