@@ -159,6 +159,14 @@ int dmrg_grouped_gemm(int ntasks, const int64_t* c_ptr, const int32_t* ldc, cons
                       const int64_t* a_ptr, const int64_t* b_ptr, const int32_t* lda, const int32_t* ldb,
                       const int32_t* kk, const int32_t* seg_flags, const double* alpha, void* cuda_stream);
 
+/* Kernel-level entry of the RDM accumulation kernel for few right-hand sides ("streams every stored
+ * 2-index operator once", HBM-bound):  E[r*ldE + c] = sum_k S[r*lds + k] * M[c*ldm + k], r < nrows, c < nc (1..8), k < K.
+ * S, M, E are DEVICE pointers (S, M 16-byte aligned, lds and ldm even); scratch is allocated and freed by the call.
+ * *ms (HOST, nullable) receives the device time of the two kernels (CUDA events on `cuda_stream`).  Used by the parity
+ * test and by bench.py's HBM probe; inside dmrg_rdm12 the same kernel serves the operator classes with nc <= 8. */
+int dmrg_stack_dots(const double* S, int64_t lds, int nrows, const double* M, int64_t ldm, int nc, int64_t K, double* E,
+                    int ldE, double* ms, void* cuda_stream);
+
 /* Device time in milliseconds (CUDA events on the call's stream around the kernel launch only, descriptor upload
  * excluded) of the most recent dmrg_grouped_gemm call in this process. */
 double dmrg_last_gemm_ms(void);

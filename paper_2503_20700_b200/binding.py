@@ -56,7 +56,7 @@ class dmrg_sweep_result(C.Structure):
 EXPORTS = ["dmrg_default_options", "dmrg_create", "dmrg_destroy", "dmrg_last_error", "dmrg_mps_import",
            "dmrg_mps_export", "dmrg_prepare_bond", "dmrg_heff_layout", "dmrg_heff_apply", "dmrg_heff_diag",
            "dmrg_heff_stats", "dmrg_sweep", "dmrg_rdm12", "dmrg_rdm_stats", "dmrg_launch_count", "dmrg_flops_total", "dmrg_device_bytes",
-           "dmrg_grouped_gemm", "dmrg_last_gemm_ms", "dmrg_fp64_probe"]
+           "dmrg_grouped_gemm", "dmrg_stack_dots", "dmrg_last_gemm_ms", "dmrg_fp64_probe"]
 
 lib.dmrg_last_error.restype = C.c_char_p
 lib.dmrg_last_error.argtypes = [C.c_void_p]
@@ -251,3 +251,13 @@ def dmrg_last_gemm_ms():
 def dmrg_flops_total(ctx):
     """Unpadded flops of every grouped-GEMM launch of the context since creation."""
     return float(lib.dmrg_flops_total(ctx))
+
+
+def dmrg_stack_dots(S_ptr, lds, nrows, M_ptr, ldm, nc, K, E_ptr, ldE, stream=None):
+    """E[r*ldE + c] = sum_k S[r*lds + k] * M[c*ldm + k] on device buffers (addresses as ints) -> device milliseconds."""
+    ms = C.c_double(0.0)
+    rc = lib.dmrg_stack_dots(C.c_void_p(S_ptr), C.c_int64(lds), int(nrows), C.c_void_p(M_ptr), C.c_int64(ldm), int(nc),
+                             C.c_int64(K), C.c_void_p(E_ptr), int(ldE), C.byref(ms), C.c_void_p(stream or 0))
+    if rc != 0:
+        raise DmrgError(rc, "dmrg_stack_dots failed")
+    return ms.value

@@ -390,6 +390,28 @@ int dmrg_rdm_stats(dmrg_ctx* ctx, double* seconds, double* bytes_streamed, doubl
     API_END
 }
 
+int dmrg_stack_dots(const double* S, int64_t lds, int nrows, const double* M, int64_t ldm, int nc, int64_t K, double* E,
+                    int ldE, double* ms, void* cuda_stream) {
+    if (!S || !M || !E || nrows < 1 || nc < 1 || nc > 8 || K < 0 || (lds & 1) || (ldm & 1) || ldE < nc) return DMRG_EINVAL;
+    if ((((uintptr_t)S) & 15) || (((uintptr_t)M) & 15)) return DMRG_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    double* scratch = nullptr;
+    const int64_t need = stack_dots_scratch(nrows, nc, K);
+    if (cudaMalloc(&scratch, sizeof(double) * (size_t)std::max<int64_t>(need, 1)) != cudaSuccess) { cudaGetLastError(); return DMRG_ENOMEM; }
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    cudaEventRecord(e0, st);
+    launch_stack_dots(S, lds, nrows, M, ldm, nc, K, E, ldE, scratch, st);
+    cudaEventRecord(e1, st);
+    const cudaError_t err = cudaStreamSynchronize(st);
+    float t = 0.f;
+    cudaEventElapsedTime(&t, e0, e1);
+    if (ms) *ms = t;
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(scratch);
+    return (err == cudaSuccess && cudaGetLastError() == cudaSuccess) ? DMRG_OK : DMRG_ECUDA;
+}
+
 static double g_last_gemm_ms = 0.0;
 double dmrg_last_gemm_ms(void) { return g_last_gemm_ms; }
 

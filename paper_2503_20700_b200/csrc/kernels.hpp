@@ -72,10 +72,13 @@ void launch_transpose(const double* in, int rows, int cols, int ld_in, double* o
 // dst[r*ld_dst + c] = alpha * src[r*ld_src + c] * (row_scale ? row_scale[r] : 1) * (col_scale ? col_scale[c] : 1)
 void launch_copy2d(double* dst, int ld_dst, const double* src, int ld_src, int rows, int cols, double alpha,
                    const double* row_scale, const double* col_scale, cudaStream_t st);
-// <A, B> = sum_ij A[i*lda+j] * B[i*ldb+j] for a batch of block pairs, out[t] += alpha[t] * <A_t, B_t> grouped by
-// target: used by the RDM accumulation (coalesced streaming of stored operators, warp-level reductions)
-struct DotPair { const double* A; const double* B; int rows, cols, lda, ldb; int target; double alpha; };
-void launch_block_dots(const DotPair* pairs, int npairs, double* out, cudaStream_t st);
+// RDM accumulation for few right-hand sides: E[r*ldE + c] = sum_k S[r*lds + k] * M[c*ldm + k], r < nrows, c < nc <= 8,
+// k < K.  Streams every row of S (a stack of stored operators) once with coalesced 16-byte loads, warp-level shuffle
+// reductions, fixed-order partial sums: HBM-bound (vec_kernels.cu).  S, M 16-byte aligned, lds, ldm even.
+// scratch: stack_dots_scratch(nrows, nc, K) doubles.
+int64_t stack_dots_scratch(int nrows, int nc, int64_t K, int64_t* span_out = nullptr, int* nspans_out = nullptr);
+void launch_stack_dots(const double* S, int64_t lds, int nrows, const double* M, int64_t ldm, int nc, int64_t K, double* E,
+                       int ldE, double* scratch, cudaStream_t st);
 
 // ---- dense SVD of a row-major [m x n] matrix (cuSOLVER gesvd; library call) -----------------------
 // U [m x r], S [r], Vt [r x n] row-major, r = min(m, n); A is destroyed.  work: opaque per-engine handle.

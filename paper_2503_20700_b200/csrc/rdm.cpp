@@ -353,6 +353,31 @@ void evaluate_group(CentreCtx& cx, ColGroup& g, const std::vector<int>& stacks, 
             part.p = nullptr;
             const size_t arena_mark = g_arena.used;
             Ed.p = g_arena.get((size_t)nrows * nc);
+            if (nc <= 8) {
+                // few right-hand sides: the HBM-bound streaming kernel (coalesced 16-byte loads of every stored operator,
+                // warp-level reductions, fixed-order partial sums) instead of the tensor-pipe GEMM
+                double* scratch = g_arena.get((size_t)stack_dots_scratch(nrows, nc, ld));
+                cudaEvent_t e0, e1;
+                cuda_check(cudaEventCreate(&e0), "event");
+                cuda_check(cudaEventCreate(&e1), "event");
+                cudaEventRecord(e0, eng.stream);
+                launch_stack_dots(stk.base, ld, nrows, Mbuf.p, ld, nc, ld, Ed.p, nc, scratch, eng.stream);
+                cudaEventRecord(e1, eng.stream);
+                eng.launches += 2;
+                eng.rdm_flops += 2.0 * nrows * (double)nc * (double)ld;
+                eng.rdm_bytes += 8.0 * ((double)nrows * ld + (double)nc * ld);
+                std::vector<double>& E = out.E[s];
+                cuda_check(cudaMemcpy2DAsync(E.data() + c0, (size_t)ncol * 8, Ed.p, (size_t)nc * 8, (size_t)nc * 8, nrows,
+                                             cudaMemcpyDeviceToHost, eng.stream), "E download");
+                cuda_check(cudaStreamSynchronize(eng.stream), "E download");
+                float ms = 0.f;
+                cudaEventElapsedTime(&ms, e0, e1);
+                eng.rdm_stream_ms += ms;
+                cudaEventDestroy(e0);
+                cudaEventDestroy(e1);
+                g_arena.used = arena_mark;
+                continue;
+            }
             GemmBatch gb, red;
             if (nsplit == 1) {
                 const int t = gb.add_task(Ed.p, nc, nrows, nc, 0);

@@ -137,36 +137,79 @@ __global__ void __launch_bounds__(256) copy2d_kernel(double* __restrict__ dst, i
     }
 }
 
-// RDM accumulation: one warp per block pair streams both blocks with coalesced loads and reduces with shuffles;
-// pairs are sorted by target and each target is owned by exactly one contiguous run handled by one CTA pass, so
-// out[target] is updated without atomics by the lane-0 thread of the first warp of the run's CTA.
-__global__ void __launch_bounds__(256) block_dots_kernel(const DotPair* __restrict__ pairs, int npairs, double* __restrict__ partial) {
-    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-    const int nwarps = (gridDim.x * blockDim.x) >> 5;
-    for (int p = warp; p < npairs; p += nwarps) {
-        const DotPair d = pairs[p];
-        double acc = 0.0;
-        if (d.lda == d.cols && d.ldb == d.cols) {
-            const int64_t total = (int64_t)d.rows * d.cols;
-            for (int64_t e = lane; e < total; e += 32) acc += d.A[e] * d.B[e];
-        } else {
-            for (int i = 0; i < d.rows; ++i)
-                for (int j = lane; j < d.cols; j += 32) acc += d.A[(size_t)i * d.lda + j] * d.B[(size_t)i * d.ldb + j];
+// RDM accumulation for few right-hand sides:
+//   E[r][c] = sum_k S[r][k] * M[c][k],   r < nrows (stored operators = rows of a stack), c < NC <= 8, k < K
+// HBM-bound: every stored operator is streamed exactly once with coalesced 16-byte loads (one warp reads 512
+// contiguous bytes of a row per instruction), the NC vectors M are staged chunk by chunk in shared memory and shared by
+// the 32 rows of the CTA, each lane keeps 2 x NC running sums, and a warp-level shuffle reduction ends every K span.
+// Partial sums of the K spans are added by a second kernel in span order (no atomics: bit-reproducible).
+constexpr int SD_WARPS = 16, SD_KC = 1024;        // 16 warps = 32 rows per CTA; 1024 doubles of every M vector per chunk
+template <int NC>
+__global__ void __launch_bounds__(SD_WARPS * 32, 2) stack_dots_kernel(const double* __restrict__ S, int64_t lds, int nrows,
+                                                                   const double* __restrict__ M, int64_t ldm, int nc, int64_t K,
+                                                                   int64_t span, int nspans, double* __restrict__ partial) {
+    extern __shared__ __align__(16) double sm[];          // [NC][SD_KC]
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int nrb = (nrows + 2 * SD_WARPS - 1) / (2 * SD_WARPS);
+    for (int64_t item = blockIdx.x; item < (int64_t)nrb * nspans; item += gridDim.x) {
+        const int rb = (int)(item % nrb), sp = (int)(item / nrb);
+        const int r0 = rb * 2 * SD_WARPS + 2 * warp;        // this warp's row pair
+        const bool v0 = r0 < nrows, v1 = r0 + 1 < nrows;
+        const double* s0 = S + (size_t)r0 * lds;
+        const double* s1 = s0 + lds;
+        const int64_t kbeg = (int64_t)sp * span, kend = kbeg + span < K ? kbeg + span : K;
+        double acc0[NC], acc1[NC];
+#pragma unroll
+        for (int c = 0; c < NC; ++c) acc0[c] = acc1[c] = 0.0;
+        for (int64_t k0 = kbeg; k0 < kend; k0 += SD_KC) {
+            __syncthreads();                                // previous chunk fully consumed
+            for (int e = threadIdx.x * 2; e < NC * SD_KC; e += SD_WARPS * 64) {
+                const int c = e / SD_KC, kk = e % SD_KC;
+                double2 m = make_double2(0.0, 0.0);
+                if (c < nc) {
+                    const int64_t k = k0 + kk;
+                    if (k + 1 < kend) m = *reinterpret_cast<const double2*>(M + (size_t)c * ldm + k);
+                    else if (k < kend) m.x = M[(size_t)c * ldm + k];
+                }
+                *reinterpret_cast<double2*>(sm + e) = m;
+            }
+            __syncthreads();
+#pragma unroll 4
+            for (int kk = lane * 2; kk < SD_KC; kk += 64) {
+                const int64_t k = k0 + kk;
+                if (k >= kend) break;
+                double2 a0 = make_double2(0.0, 0.0), a1 = make_double2(0.0, 0.0);
+                if (k + 1 < kend) {
+                    if (v0) a0 = *reinterpret_cast<const double2*>(s0 + k);
+                    if (v1) a1 = *reinterpret_cast<const double2*>(s1 + k);
+                } else {
+                    if (v0) a0.x = s0[k];
+                    if (v1) a1.x = s1[k];
+                }
+#pragma unroll
+                for (int c = 0; c < NC; ++c) {
+                    const double2 m = *reinterpret_cast<const double2*>(sm + c * SD_KC + kk);
+                    acc0[c] = fma(a0.x, m.x, fma(a0.y, m.y, acc0[c]));
+                    acc1[c] = fma(a1.x, m.x, fma(a1.y, m.y, acc1[c]));
+                }
+            }
         }
-        acc = warp_sum(acc);
-        if (lane == 0) partial[p] = d.alpha * acc;
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            const double t0 = warp_sum(acc0[c]), t1 = warp_sum(acc1[c]);
+            if (lane == 0 && c < nc) {
+                if (v0) partial[((size_t)sp * nrows + r0) * nc + c] = t0;
+                if (v1) partial[((size_t)sp * nrows + r0 + 1) * nc + c] = t1;
+            }
+        }
     }
 }
-// out[target] += sum of partial[p] over the pairs of that target, in pair order (one thread per target run)
-__global__ void block_dots_reduce(const DotPair* __restrict__ pairs, int npairs, const double* __restrict__ partial,
-                                  double* __restrict__ out) {
-    const int p = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= npairs) return;
-    if (p > 0 && pairs[p - 1].target == pairs[p].target) return;     // not the head of a run
-    const int tgt = pairs[p].target;
+__global__ void stack_dots_reduce(const double* __restrict__ partial, int nrows, int nc, int nspans, double* __restrict__ E, int ldE) {
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= nrows * nc) return;
     double s = 0.0;
-    for (int q = p; q < npairs && pairs[q].target == tgt; ++q) s += partial[q];
-    out[tgt] += s;
+    for (int sp = 0; sp < nspans; ++sp) s += partial[(size_t)sp * nrows * nc + idx];
+    E[(size_t)(idx / nc) * ldE + idx % nc] = s;
 }
 
 int grid_for(int64_t n, int threads) {
@@ -177,8 +220,6 @@ int grid_for(int64_t n, int threads) {
 }
 
 double* g_partial = nullptr;    // scratch of the two-stage reductions (COMBINE_MAX x RED_BLOCKS doubles)
-double* g_pair_partial = nullptr;
-size_t g_pair_cap = 0;
 
 }  // namespace
 
@@ -223,17 +264,42 @@ void launch_copy2d(double* dst, int ldd, const double* src, int lds, int rows, i
     if (rows <= 0 || cols <= 0) return;
     copy2d_kernel<<<grid_for((int64_t)rows * cols, 256), 256, 0, st>>>(dst, ldd, src, lds, rows, cols, alpha, rs, cs);
 }
-void launch_block_dots(const DotPair* pairs, int npairs, double* out, cudaStream_t st) {
-    if (npairs <= 0) return;
-    if ((size_t)npairs > g_pair_cap) {
-        if (g_pair_partial) cudaFree(g_pair_partial);
-        g_pair_cap = (size_t)npairs * 2;
-        cudaMalloc(&g_pair_partial, sizeof(double) * g_pair_cap);
+int64_t stack_dots_scratch(int nrows, int nc, int64_t K, int64_t* span_out, int* nspans_out) {
+    // K spans: enough work items (row blocks x spans) for ~8 per resident CTA, at least one chunk each
+    const int nrb = (nrows + 2 * SD_WARPS - 1) / (2 * SD_WARPS);
+    const int64_t nch = K > 0 ? (K + SD_KC - 1) / SD_KC : 1;   // K == 0: one empty span (E = 0)
+    int64_t want = (148 * 2 * 8 + nrb - 1) / nrb;
+    if (want < 1) want = 1;
+    if (want > nch) want = nch;
+    int64_t per = (nch + want - 1) / want;                  // chunks per span
+    const int64_t span = per * SD_KC;
+    const int nspans = K > 0 ? (int)((K + span - 1) / span) : 1;
+    if (span_out) *span_out = span;
+    if (nspans_out) *nspans_out = nspans;
+    return (int64_t)nspans * nrows * nc;
+}
+void launch_stack_dots(const double* S, int64_t lds, int nrows, const double* M, int64_t ldm, int nc, int64_t K, double* E,
+                       int ldE, double* scratch, cudaStream_t st) {
+    if (nrows <= 0 || nc <= 0 || nc > 8) return;
+    int64_t span = 0;
+    int nspans = 0;
+    stack_dots_scratch(nrows, nc, K, &span, &nspans);
+    const int nrb = (nrows + 2 * SD_WARPS - 1) / (2 * SD_WARPS);
+    const int64_t items = (int64_t)nrb * nspans;
+    const int grid = (int)(items < 148 * 2 * 4 ? items : 148 * 2 * 4);
+    const int NCt = nc <= 1 ? 1 : (nc <= 2 ? 2 : (nc <= 4 ? 4 : 8));
+    const int smem = NCt * SD_KC * (int)sizeof(double);
+    static bool configured = false;
+    if (!configured) {
+        cudaFuncSetAttribute(stack_dots_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 8 * SD_KC * 8);
+        configured = true;
     }
-    int blocks = (npairs + 7) / 8;
-    if (blocks > RED_BLOCKS * 2) blocks = RED_BLOCKS * 2;
-    block_dots_kernel<<<blocks, 256, 0, st>>>(pairs, npairs, g_pair_partial);
-    block_dots_reduce<<<(npairs + 255) / 256, 256, 0, st>>>(pairs, npairs, g_pair_partial, out);
+    if (K <= 0) { cudaMemsetAsync(scratch, 0, sizeof(double) * (size_t)nspans * nrows * nc, st); }
+    else if (NCt == 1) stack_dots_kernel<1><<<grid, SD_WARPS * 32, smem, st>>>(S, lds, nrows, M, ldm, nc, K, span, nspans, scratch);
+    else if (NCt == 2) stack_dots_kernel<2><<<grid, SD_WARPS * 32, smem, st>>>(S, lds, nrows, M, ldm, nc, K, span, nspans, scratch);
+    else if (NCt == 4) stack_dots_kernel<4><<<grid, SD_WARPS * 32, smem, st>>>(S, lds, nrows, M, ldm, nc, K, span, nspans, scratch);
+    else stack_dots_kernel<8><<<grid, SD_WARPS * 32, smem, st>>>(S, lds, nrows, M, ldm, nc, K, span, nspans, scratch);
+    stack_dots_reduce<<<(nrows * nc + 255) / 256, 256, 0, st>>>(scratch, nrows, nc, nspans, E, ldE);
 }
 
 }  // namespace dmrg

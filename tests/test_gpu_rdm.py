@@ -86,3 +86,26 @@ def test_rdm12_config1_truncated_sweep_vs_oracle(lib):
     _invariants(g, G, n)
     e_rdm = np.einsum("pq,pq->", cfg["h"], g) + 0.5 * np.einsum("pqrs,pqrs->", cfg["eri"], G)
     assert e_rdm >= r["energy_min"] - 1e-9                           # <Psi|H|Psi> of the truncated MPS (reading S20)
+
+
+@pytest.mark.parametrize("nrows,nc,K", [(1, 1, 1), (5, 3, 77), (33, 8, 1025), (64, 2, 4096 + 3), (70, 5, 2 * 1024 * 9 + 1), (3, 8, 0)])
+def test_stack_dots_kernel_matches_definition(lib, nrows, nc, K):
+    """RDM accumulation kernel for few right-hand sides against its definition E = S M^T (numpy, FP64): ragged row
+    counts, K tails (odd, below / above one chunk, several spans), every template width."""
+    import torch
+    rng = np.random.default_rng(nrows * 1000 + nc)
+    lds = K + (K & 1) + 2
+    ldm = K + (K & 1) + 4
+    S = rng.normal(size=(nrows, lds))
+    M = rng.normal(size=(nc, ldm))
+    Sd, Md = torch.tensor(S, device="cuda"), torch.tensor(M, device="cuda")
+    ldE = nc + 1
+    Ed = torch.full((nrows, ldE), 7.0, dtype=torch.float64, device="cuda")
+    ms = lib.dmrg_stack_dots(Sd.data_ptr(), lds, nrows, Md.data_ptr(), ldm, nc, K, Ed.data_ptr(), ldE,
+                             torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert ms >= 0.0
+    E = Ed.cpu().numpy()
+    ref = S[:, :K] @ M[:, :K].T
+    assert np.abs(E[:, :nc] - ref).max() <= 1e-12 * max(1.0, np.abs(ref).max()) * max(1.0, np.sqrt(K))
+    assert np.all(E[:, nc:] == 7.0)
