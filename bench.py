@@ -387,6 +387,21 @@ def run_ours(args):
         pr["note"] = "kinds 0-2: 3 CTAs x 4 warps per SM, 16 independent DMMA.8x8x4 (or 32 DFMA) per warp per iteration"
         line["fp64_probe"] = pr
         roof["frac_of_dmma_probe"] = achieved / pr["dmma_regs"]["tflops"]
+        # HBM-bound RDM accumulation kernel (row a6) at a config-4-like shape: 1024 stored operators of 2^20 doubles each
+        # (8.6 GB, larger than L2) against nc right-hand sides; bytes = every operator once + the nc vectors
+        nrows, K = 1024, 1 << 20
+        S = torch.randn(nrows, K, device=dev, dtype=torch.float64)
+        sp = {}
+        for nc in (1, 4, 8):
+            M = torch.randn(nc, K, device=dev, dtype=torch.float64)
+            E = torch.empty(nrows, nc, device=dev, dtype=torch.float64)
+            ms = min(P.dmrg_stack_dots(S.data_ptr(), K, nrows, M.data_ptr(), K, nc, K, E.data_ptr(), nc,
+                                       torch.cuda.current_stream().cuda_stream) for _ in range(4))
+            gb = 8.0 * (nrows * K + nc * K) / 1e9
+            sp["nc%d" % nc] = {"ms": ms, "gbytes": gb, "gbs": gb / ms * 1e3, "frac_of_hbm": gb / ms * 1e3 / peaks["hbm"]}
+        sp["note"] = "dmrg_stack_dots: E = S M^T, 1024 x 2^20 doubles streamed once per call; hbm peak %s %.0f GB/s" % (peaks["src"], peaks["hbm"])
+        line["rdm_stream_probe"] = sp
+        del S
     if args.extras:
         line["extras"] = time_small_extras(P, torch, peaks, args.extras)
     if args.cpu_baseline and world == 1:
