@@ -378,6 +378,7 @@ def run_ours(args):
                     "ms_per_step": e2e_s * 1e3},
             "gpu_launches": int(launches), "clocks": clocks, "roofline": roof}
     if args.probe:
+        torch.cuda.profiler.start()                  # the timed region ended with profiler.stop(): let ncu see the probes
         # the ceilings the roofline fraction should be read against, measured in the same process on the same box
         pr = {}
         for name, kind, kw in (("dmma_regs", 0, {}), ("dfma_regs", 1, {}), ("dmma_lds", 2, {}),
@@ -402,6 +403,7 @@ def run_ours(args):
         sp["note"] = "dmrg_stack_dots: E = S M^T, 1024 x 2^20 doubles streamed once per call; hbm peak %s %.0f GB/s" % (peaks["src"], peaks["hbm"])
         line["rdm_stream_probe"] = sp
         del S
+        torch.cuda.profiler.stop()
     if args.extras:
         line["extras"] = time_small_extras(P, torch, peaks, args.extras)
     if args.cpu_baseline and world == 1:
