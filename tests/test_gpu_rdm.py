@@ -109,3 +109,23 @@ def test_stack_dots_kernel_matches_definition(lib, nrows, nc, K):
     ref = S[:, :K] @ M[:, :K].T
     assert np.abs(E[:, :nc] - ref).max() <= 1e-12 * max(1.0, np.abs(ref).max()) * max(1.0, np.sqrt(K))
     assert np.all(E[:, nc:] == 7.0)
+
+
+@pytest.mark.parametrize("cid,D", [(2, 12), (3, 12)])
+def test_rdm12_config_geometries_small_D_vs_oracle(lib, cid, D):
+    """1-/2-RDM element by element against the oracle on the Hamiltonians and chain lengths of BASELINE configs 2
+    (coronene, k = 24) and 3 (Fe-S-like, k = 20, N = 30 > k), at a bond dimension the plain oracle pass finishes in
+    about a minute (the full D = 512 / 1024 oracle pass would take hours; the GPU pass at full D is checked by its
+    invariants in bench.py and test_rdm12_after_sweep_energy_and_fci)."""
+    cfg = make_config(cid)
+    k, n = cfg["k"], cfg["n_elec"]
+    mps = random_mps(k, n, 0, D, seed=900 + cid, gauge="R")
+    g0, G0 = odmrg.rdm12(cfg["h"], cfg["eri"], mps, True)
+    ctx = lib.dmrg_create(k, n, 0, cfg["h"], cfg["eri"])
+    try:
+        lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, 0)
+        g, G = lib.dmrg_rdm12(ctx, k, True)
+    finally:
+        lib.dmrg_destroy(ctx)
+    assert np.abs(g - g0).max() <= TOL and np.abs(G - G0).max() <= TOL
+    _invariants(g, G, n)
