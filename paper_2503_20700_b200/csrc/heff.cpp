@@ -7,6 +7,11 @@
 // block) or T = X O_R^T, whichever order needs fewer flops for the (term, block) pair.  Phase 2 gives every output
 // block to one task that sums its contributions  Y += c T O_R^T  /  Y += c O_L T  as one K-concatenated GEMM: no
 // atomics, fixed summation order.  Terms are processed in chunks bounded by the intermediate buffer.
+//
+// The descriptors (which triples contribute, signs, intermediates, segment lists, tiles, diagonal items, accounting)
+// are enumerated on the device by heff_maps.cu from small uploaded tables (build_maps_device below); the host loop in
+// build_heff is the reference builder kept for A/B tests (DMRG_B200_HOST_MAPS=1).  heff_apply runs the chunks as a
+// two-stream pipeline with double-buffered intermediates and split-K partial sums.
 #include <algorithm>
 #include <cassert>
 #include <cstdlib>

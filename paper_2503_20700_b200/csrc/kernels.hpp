@@ -1,5 +1,5 @@
-// Launchers of the sm_100a CUDA kernels (the only place tensor arithmetic happens).  Implemented in seg_gemm.cu,
-// vec_kernels.cu and linalg.cu.  All pointers are device pointers unless a name ends in _host.
+// Launchers of the sm_100a CUDA kernels (the only place tensor arithmetic happens).  Implemented in seg_gemm_tma.cu,
+// seg_gemm.cu, vec_kernels.cu, linalg.cu and probe.cu (the integer block-map kernels are in heff_maps.cu / maps.hpp).  All pointers are device pointers unless a name ends in _host.
 #pragma once
 #include <cuda_runtime_api.h>
 
