@@ -39,6 +39,24 @@ typedef struct dmrg_options {
     int32_t keep_env_stack;       /* default 1: keep every environment block (needed by sweeps); 0: prepare_bond
                                      keeps only the two blocks of the prepared bond (large-D single-bond runs)  */
     int64_t workspace_bytes;      /* default 0 = automatic: cap of the intermediate (T) buffer of H_eff psi   */
+    /* Environment stack of dmrg_sweep (BASELINE configs 4-5: "operator storage sized to fit 180 GB HBM"; SURVEY.md 7
+     * hard part 5).  One pass consumes the blocks the previous pass produced; only every env_stride-th block is kept
+     * (a checkpoint), the blocks in between are recomputed from it when the pass reaches them; with host_spill the
+     * checkpoints are moved to pinned host memory by asynchronous copies and fetched back when needed.  Results do not
+     * depend on these settings (the recomputed blocks are bit-identical). */
+    int64_t hbm_budget_bytes;     /* default 0 = automatic (55 % of the free device memory): bytes the stack may hold */
+    int64_t host_budget_bytes;    /* default 0 = automatic (96 GiB): pinned host bytes for spilled checkpoints        */
+    int32_t host_spill;           /* default 0; 1: checkpoints may be spilled to pinned host memory                    */
+    int32_t env_stride;           /* default 0 = automatic from the budgets; 1 = keep every block; s: every s-th       */
+    /* Dynamic block state selection: dbss_eps > 0 keeps, at every bond, the fewest states
+     * whose discarded weight is <= dbss_eps, at least dbss_dmin and at most the D passed to dmrg_sweep (D_max).       */
+    double dbss_eps;              /* default 0 = fixed D                                                               */
+    int32_t dbss_dmin;            /* default 0                                                                         */
+    int32_t split_k;              /* default 0 = automatic: split-K parts (1..16) of phase 2 of H_eff psi              */
+    int32_t svd_qr;               /* default 0: one-sided Jacobi SVD (cuSOLVER gesvdj, gesvd fallback); 1: gesvd       */
+    int32_t host_maps;            /* default 0: block maps built on the device; 1: host reference builder (A/B tests)  */
+    int32_t generic_gemm;         /* default 0; 1: always the cp.async GEMM kernel instead of the bulk-copy one (A/B)  */
+    int32_t reserved0;
 } dmrg_options;
 
 /* Neutral MPS exchange format (host memory, caller-owned, flat arrays).
@@ -118,7 +136,7 @@ int dmrg_heff_layout(dmrg_ctx* ctx, int i, int64_t* nnz, int32_t* nblocks, dmrg_
  * cuda_stream: a cudaStream_t (NULL = default stream); device buffers are used in place, asynchronously on that
  * stream; host buffers are copied in and out and the call returns after completion.  Never modifies the MPS. */
 int dmrg_heff_apply(dmrg_ctx* ctx, int i, const double* x, double* y, int where, void* cuda_stream);
-/* diag(H_eff) at the prepared bond (Davidson preconditioner), same layout and `where` semantics. */
+/* diag(H_eff) at the prepared bond (Davidson preconditioner), same layout, `where` and stream semantics. */
 int dmrg_heff_diag(dmrg_ctx* ctx, int i, double* d, int where, void* cuda_stream);
 /* Flop and byte accounting of one H_eff psi at the prepared bond (D3): f_alg = canonical algorithmic
  * flops with true sector dimensions, f_exec = flops of the GEMMs actually issued (unpadded), b_alg = 8 x (nnz of
@@ -131,9 +149,22 @@ int dmrg_heff_stats(dmrg_ctx* ctx, int i, double* f_alg, double* f_exec, double*
  * Returns DMRG_ENOCONV (warning) if any Davidson hit max_iter. */
 int dmrg_sweep(dmrg_ctx* ctx, int D, dmrg_sweep_result* result, dmrg_bond_record* records);
 
+/* Phase timers and environment-stack accounting of the last dmrg_sweep call (seconds per phase).
+ * seconds_environments = restore + regrow + the initial right stack; seconds_spill_wait = time the host waited for an
+ * asynchronous spill copy before it could free the device copy (0 when the copy was hidden behind the bond's Davidson). */
+typedef struct dmrg_sweep_stats_t {
+    double seconds_environments, seconds_restore, seconds_regrow, seconds_spill_wait;
+    double seconds_maps, seconds_davidson, seconds_matvec, seconds_split, seconds_renormalise;
+    double bytes_spilled, bytes_restored;
+    int64_t peak_device_bytes, host_pool_bytes, est_stack_bytes, est_max_block_bytes;
+    int32_t env_stride, host_spill;
+} dmrg_sweep_stats_t;
+int dmrg_sweep_stats(dmrg_ctx* ctx, dmrg_sweep_stats_t* out);
+
 /* gamma (k*k) and Gamma (k^4, nullable -> 1-RDM only) of the normalised current MPS (readings S2, S20):
  * gamma_pq = <E_pq>, Gamma_pqrs = <sum_ss' a+_ps a+_rs' a_ss' a_qs> at ((p*k+q)*k+r)*k+s.  Output buffers host or
- * device per `where`. */
+ * device per `where`; device buffers are written on `cuda_stream` after its pending work, and the call returns when
+ * the results are in place. */
 int dmrg_rdm12(dmrg_ctx* ctx, double* gamma, double* Gamma, int where, void* cuda_stream);
 
 /* Timing / accounting of the last dmrg_rdm12 call: seconds of the whole pass, bytes of operator storage streamed by

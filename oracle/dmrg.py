@@ -167,31 +167,67 @@ def empty_block(side, k, mps):
 # ----------------------------------------------------------------------------------------------------------------
 # complementary two-index operators of a block from its normal operators, by definition (C3 step 1)
 # ----------------------------------------------------------------------------------------------------------------
+def _stacked(blk, kind):
+    """All stored operators of one kind on a block, grouped by label shift and laid side by side per in-sector:
+    {dq: (keys, {in_idx: (out_idx, array[n_ops, d_out, d_in], present[n_ops])})}.  Built once per block (its operators
+    never change after construction).  Only a container: it lets the defining sums of compl_P / compl_Q below run as
+    one library contraction (np.tensordot over the operator index) instead of a Python loop of block additions."""
+    cache = blk.__dict__.setdefault("_stacks", {})
+    if kind not in cache:
+        groups = {}
+        for key, op in blk.ops.items():
+            if key[0] == kind:
+                groups.setdefault(op.dq, []).append(key)
+        out = {}
+        for dq, keys in groups.items():
+            arrs = {}
+            for i in sorted({i for key in keys for i in blk.ops[key].blocks}):
+                first = next(blk.ops[key].blocks[i] for key in keys if i in blk.ops[key].blocks)
+                st = np.zeros((len(keys),) + first[1].shape)
+                present = np.zeros(len(keys), dtype=bool)
+                for n, key in enumerate(keys):
+                    if i in blk.ops[key].blocks:
+                        assert blk.ops[key].blocks[i][0] == first[0]
+                        st[n] = blk.ops[key].blocks[i][1]
+                        present[n] = True
+                arrs[i] = (first[0], st, present)
+            out[dq] = (keys, arrs)
+        cache[kind] = out
+    return cache[kind]
+
+
 def compl_P(blk, ham, P, Q):
-    """P_PQ^X = sum_{R,S in X} v_PQRS a_R a_S = sum_{R<S in X} (v_PQSR - v_PQRS) (A_RS)^T."""
+    """P_PQ^X = sum_{R,S in X} v_PQRS a_R a_S = sum_{R<S in X} (v_PQSR - v_PQRS) (A_RS)^T  (C3 step 1); the sum over
+    the stored A_RS (those whose shift matches) is one tensordot per block."""
     g = blk.sgn()
     dq = (-2, -((1 if P % 2 == 0 else -1) + (1 if Q % 2 == 0 else -1)))
     out = BlockOp((g * dq[0], g * dq[1]), 0)
-    ins = blk.inside()
-    for a_, R in enumerate(ins):
-        for S in ins[a_ + 1:]:
-            c = ham.v(P, Q, S, R) - ham.v(P, Q, R, S)
-            if c != 0.0:
-                out.add(c, blk.ops[("A", R, S)].T())
+    entry = _stacked(blk, "A").get((-out.dq[0], -out.dq[1]))          # A_RS carries the opposite label shift
+    if entry is None:
+        return out
+    keys, arrs = entry
+    c = np.array([ham.v(P, Q, S, R) - ham.v(P, Q, R, S) for (_, R, S) in keys])
+    nz = c != 0.0
+    for i, (o, st, present) in arrs.items():
+        if np.any(nz & present):
+            out.blocks[o] = (i, np.ascontiguousarray(np.tensordot(c, st, axes=1).T))
     return out
 
 
 def compl_Q(blk, ham, P, S):
-    """Q_PS^X = sum_{Q,R in X} (v_PQRS - v_PQSR) a+_Q a_R."""
+    """Q_PS^X = sum_{Q,R in X} (v_PQRS - v_PQSR) a+_Q a_R  (C3 step 1); one tensordot over the stored B_QR per block."""
     g = blk.sgn()
     dq = (0, -(1 if P % 2 == 0 else -1) + (1 if S % 2 == 0 else -1))
     out = BlockOp((g * dq[0], g * dq[1]), 0)
-    ins = blk.inside()
-    for Q in ins:
-        for R in ins:
-            c = ham.w(P, Q, R, S)
-            if c != 0.0:
-                out.add(c, blk.ops[("B", Q, R)])
+    entry = _stacked(blk, "B").get(out.dq)
+    if entry is None:
+        return out
+    keys, arrs = entry
+    c = np.array([ham.w(P, Q, R, S) for (_, Q, R) in keys])
+    nz = c != 0.0
+    for i, (o, st, present) in arrs.items():
+        if np.any(nz & present):
+            out.blocks[i] = (o, np.tensordot(c, st, axes=1))
     return out
 
 
@@ -569,6 +605,28 @@ class Heff:
 
     def apply(self, x):
         return blocks_to_flat(self.layout, self.nnz, self.apply_blocks(flat_to_blocks(self.layout, x)))
+
+    def gemm_flops(self):
+        """Flops of the matrix products one apply() executes, counted by walking the term list with the loop
+        structure of apply_blocks: (ml @ x) @ mr^T = 2 d_lo d_li d_ri + 2 d_lo d_ri d_ro per (term, site-state pair,
+        block), and the same again with the transposed factors for terms that add their Hermitian conjugate.
+        Integer bookkeeping only - no arithmetic of the method is done here."""
+        f = 0
+        for (coef, E, F, hc) in self.terms:
+            for (ao, ai), OL in E.grid.items():
+                for (bo, bi), OR in F.grid.items():
+                    for li, (lo, ml) in OL.blocks.items():
+                        kin = (li, ai, bi)
+                        if kin not in self.by_key:
+                            continue
+                        ri, m_in, n_in = self.by_key[kin]
+                        if ri not in OR.blocks or (lo, ao, bo) not in self.by_key:
+                            continue
+                        m_out, n_out = ml.shape[0], OR.blocks[ri][1].shape[0]
+                        f += 2 * m_out * m_in * n_in + 2 * m_out * n_in * n_out
+                        if hc:
+                            f += 2 * m_in * m_out * n_out + 2 * m_in * n_out * n_in
+        return float(f)
 
     def diagonal(self):
         """diag(H_eff) for the Davidson preconditioner: terms with all four factors on the diagonal."""

@@ -25,7 +25,10 @@ DMRG_HOST, DMRG_DEVICE = 0, 1
 class dmrg_options(C.Structure):
     _fields_ = [("davidson_tol", C.c_double), ("davidson_max_iter", C.c_int32), ("davidson_max_subspace", C.c_int32),
                 ("sv_floor", C.c_double), ("cluster_rel_gap", C.c_double), ("device_id", C.c_int32),
-                ("keep_env_stack", C.c_int32), ("workspace_bytes", C.c_int64)]
+                ("keep_env_stack", C.c_int32), ("workspace_bytes", C.c_int64),
+                ("hbm_budget_bytes", C.c_int64), ("host_budget_bytes", C.c_int64), ("host_spill", C.c_int32),
+                ("env_stride", C.c_int32), ("dbss_eps", C.c_double), ("dbss_dmin", C.c_int32), ("split_k", C.c_int32),
+                ("svd_qr", C.c_int32), ("host_maps", C.c_int32), ("generic_gemm", C.c_int32), ("reserved0", C.c_int32)]
 
 
 class dmrg_mps_blob(C.Structure):
@@ -55,7 +58,7 @@ class dmrg_sweep_result(C.Structure):
 
 EXPORTS = ["dmrg_default_options", "dmrg_create", "dmrg_destroy", "dmrg_last_error", "dmrg_mps_import",
            "dmrg_mps_export", "dmrg_prepare_bond", "dmrg_heff_layout", "dmrg_heff_apply", "dmrg_heff_diag",
-           "dmrg_heff_stats", "dmrg_sweep", "dmrg_rdm12", "dmrg_rdm_stats", "dmrg_launch_count", "dmrg_flops_total", "dmrg_device_bytes",
+           "dmrg_heff_stats", "dmrg_sweep", "dmrg_sweep_stats", "dmrg_rdm12", "dmrg_rdm_stats", "dmrg_launch_count", "dmrg_flops_total", "dmrg_device_bytes",
            "dmrg_grouped_gemm", "dmrg_stack_dots", "dmrg_last_gemm_ms", "dmrg_fp64_probe"]
 
 lib.dmrg_last_error.restype = C.c_char_p
@@ -194,8 +197,30 @@ def dmrg_sweep(ctx, D, k):
                 warnings=res.warnings, status=rc, bonds=bonds)
 
 
-def dmrg_rdm12(ctx, k, want_2rdm=True):
-    """-> (gamma [k,k], Gamma [k,k,k,k] or None) as numpy arrays."""
+class dmrg_sweep_stats_t(C.Structure):
+    _fields_ = [(n, C.c_double) for n in ("seconds_environments", "seconds_restore", "seconds_regrow",
+                                          "seconds_spill_wait", "seconds_maps", "seconds_davidson", "seconds_matvec",
+                                          "seconds_split", "seconds_renormalise", "bytes_spilled", "bytes_restored")] + \
+               [(n, C.c_int64) for n in ("peak_device_bytes", "host_pool_bytes", "est_stack_bytes", "est_max_block_bytes")] + \
+               [("env_stride", C.c_int32), ("host_spill", C.c_int32)]
+
+
+def dmrg_sweep_stats(ctx):
+    """Phase seconds and environment-stack accounting of the last dmrg_sweep -> dict."""
+    st = dmrg_sweep_stats_t()
+    _check(ctx, lib.dmrg_sweep_stats(ctx, C.byref(st)))
+    return dict((f, getattr(st, f)) for f, _ in dmrg_sweep_stats_t._fields_)
+
+
+def dmrg_rdm12(ctx, k, want_2rdm=True, out=None):
+    """-> (gamma [k,k], Gamma [k,k,k,k] or None) as numpy arrays; with out = (gamma, Gamma) torch CUDA tensors the
+    results are written to those device buffers (on torch's current stream) and returned."""
+    if out is not None:
+        g, G = out
+        pg, where, stream = _vec(g)
+        pG = _vec(G)[0] if (want_2rdm and G is not None) else None
+        _check(ctx, lib.dmrg_rdm12(ctx, pg, pG, where, stream))
+        return g, G
     g = np.zeros((k, k))
     G = np.zeros((k, k, k, k)) if want_2rdm else None
     _check(ctx, lib.dmrg_rdm12(ctx, _ptr(g), _ptr(G) if want_2rdm else None, DMRG_HOST, None))

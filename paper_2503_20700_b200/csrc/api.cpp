@@ -49,7 +49,8 @@ HeffPlan::~HeffPlan() {
 #define API_BEGIN(ctx)                                   \
     if (!(ctx)) return DMRG_EINVAL;                      \
     Engine& eng = (ctx)->eng;                            \
-    try {
+    try {                                                \
+        cuda_check(cudaSetDevice(eng.opt.device_id), "cudaSetDevice");
 #define API_END                                          \
     }                                                    \
     catch (const Error& e) { eng.last_error = e.what(); return e.code; }                 \
@@ -74,6 +75,9 @@ void dmrg_default_options(dmrg_options* o) {
     o->device_id = 0;
     o->keep_env_stack = 1;
     o->workspace_bytes = 0;
+    o->hbm_budget_bytes = 0; o->host_budget_bytes = 0; o->host_spill = 0; o->env_stride = 0;
+    o->dbss_eps = 0.0; o->dbss_dmin = 0; o->split_k = 0; o->svd_qr = 0; o->host_maps = 0; o->generic_gemm = 0;
+    o->reserved0 = 0;
 }
 
 int dmrg_create(dmrg_ctx** out, int k, int n_elec, int two_sz, const double* h, const double* eri,
@@ -100,23 +104,29 @@ int dmrg_create(dmrg_ctx** out, int k, int n_elec, int two_sz, const double* h, 
             eng.opt.device_id = opt->device_id;
             eng.opt.workspace_bytes = opt->workspace_bytes;
             eng.keep_env_stack = opt->keep_env_stack != 0;
+            eng.opt.hbm_budget_bytes = opt->hbm_budget_bytes; eng.opt.host_budget_bytes = opt->host_budget_bytes;
+            eng.opt.host_spill = opt->host_spill; eng.opt.env_stride = opt->env_stride;
+            eng.opt.dbss_eps = opt->dbss_eps; eng.opt.dbss_dmin = opt->dbss_dmin;
+            eng.opt.split_k = opt->split_k; eng.opt.svd_qr = opt->svd_qr;
+            eng.host_maps = opt->host_maps != 0; eng.force_generic_gemm = opt->generic_gemm != 0;
         }
         if (eng.opt.davidson_max_subspace < 2 || eng.opt.davidson_max_subspace > COMBINE_MAX ||
-            eng.opt.davidson_max_iter < 1 || !(eng.opt.davidson_tol > 0)) { delete ctx; return DMRG_EINVAL; }
+            eng.opt.davidson_max_iter < 1 || !(eng.opt.davidson_tol > 0) || eng.opt.env_stride < 0 ||
+            eng.opt.split_k < 0 || eng.opt.split_k > 16 || eng.opt.dbss_eps < 0 || eng.opt.dbss_dmin < 0 ||
+            eng.opt.hbm_budget_bytes < 0 || eng.opt.host_budget_bytes < 0) { delete ctx; return DMRG_EINVAL; }
         int ndev = 0;
         if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= eng.opt.device_id) { delete ctx; return DMRG_ECUDA; }
         cuda_check(cudaSetDevice(eng.opt.device_id), "cudaSetDevice");
         cuda_check(cudaStreamCreateWithFlags(&eng.stream, cudaStreamNonBlocking), "cudaStreamCreate");
         cuda_check(cudaStreamCreateWithFlags(&eng.stream2, cudaStreamNonBlocking), "cudaStreamCreate");
+        cuda_check(cudaStreamCreateWithFlags(&eng.copy_stream, cudaStreamNonBlocking), "cudaStreamCreate");
         eng.k = k; eng.n_elec = n_elec; eng.two_sz = two_sz;
         eng.bsw = (k >= 3) ? (k - 3) / 2 : -1;
         eng.ham.k = k;
         eng.ham.h.assign(h, h + (size_t)k * k);
         eng.ham.eri.assign(eri, eri + (size_t)k * k * k * k);
-        eng.svd = svd_create(eng.stream);
-        { const char* g = std::getenv("DMRG_B200_GENERIC_GEMM"); eng.force_generic_gemm = g && g[0] == '1'; }
-        { const char* g = std::getenv("DMRG_B200_TRACE"); eng.trace = g && g[0] == '1'; }
-        { const char* g = std::getenv("DMRG_B200_HOST_MAPS"); eng.host_maps = g && g[0] == '1'; }
+        eng.svd = svd_create(eng.stream, eng.opt.svd_qr == 0);
+        { const char* g = std::getenv("DMRG_B200_TRACE"); eng.trace = g && g[0] == '1'; }   // diagnostics only: per-launch times on stderr
     } catch (...) {
         delete ctx;
         return DMRG_ECUDA;
@@ -128,13 +138,14 @@ int dmrg_create(dmrg_ctx** out, int k, int n_elec, int two_sz, const double* h, 
 int dmrg_destroy(dmrg_ctx* ctx) {
     if (!ctx) return DMRG_EINVAL;
     Engine& eng = ctx->eng;
-    eng.plan.reset();
-    eng.L.clear();
-    eng.R.clear();
+    cudaSetDevice(eng.opt.device_id);
+    eng.invalidate();
+    eng.host_pool.clear();
     eng.mps.sites.clear();
     if (eng.svd) svd_destroy(eng.svd);
     if (eng.stream) cudaStreamDestroy(eng.stream);
     if (eng.stream2) cudaStreamDestroy(eng.stream2);
+    if (eng.copy_stream) cudaStreamDestroy(eng.copy_stream);
     delete ctx;
     return DMRG_OK;
 }
@@ -299,15 +310,26 @@ int dmrg_heff_apply(dmrg_ctx* ctx, int i, const double* x, double* y, int where,
 
 int dmrg_heff_diag(dmrg_ctx* ctx, int i, double* d, int where, void* cuda_stream) {
     API_BEGIN(ctx)
-    (void)cuda_stream;
     if (int rc = need_plan(eng, i)) return rc;
     if (!d) return fail(eng, DMRG_EINVAL, "heff_diag: null vector");
     HeffPlan& p = *eng.plan;
     if (where == DMRG_HOST) {
         heff_diag(p, p.ybuf.p, eng);
         cuda_check(cudaMemcpyAsync(d, p.ybuf.p, (size_t)p.nnz * 8, cudaMemcpyDeviceToHost, eng.stream), "diag download");
-    } else heff_diag(p, d, eng);
-    cuda_check(cudaStreamSynchronize(eng.stream), "heff_diag");
+        cuda_check(cudaStreamSynchronize(eng.stream), "heff_diag");
+    } else if (where == DMRG_DEVICE) {
+        // same ordering as dmrg_heff_apply: the library stream starts after the caller's pending work on `d` and the
+        // caller's stream continues after the kernel; asynchronous
+        cudaStream_t cs = (cudaStream_t)cuda_stream;
+        cudaEvent_t ev;
+        cuda_check(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming), "event");
+        cuda_check(cudaEventRecord(ev, cs), "event record");
+        cuda_check(cudaStreamWaitEvent(eng.stream, ev, 0), "stream wait");
+        heff_diag(p, d, eng);
+        cuda_check(cudaEventRecord(ev, eng.stream), "event record");
+        cuda_check(cudaStreamWaitEvent(cs, ev, 0), "stream wait");
+        cuda_check(cudaEventDestroy(ev), "event destroy");
+    } else return fail(eng, DMRG_EINVAL, "heff_diag: bad `where`");
     return DMRG_OK;
     API_END
 }
@@ -362,19 +384,36 @@ int dmrg_sweep(dmrg_ctx* ctx, int D, dmrg_sweep_result* result, dmrg_bond_record
     API_END
 }
 
+int dmrg_sweep_stats(dmrg_ctx* ctx, dmrg_sweep_stats_t* out) {
+    API_BEGIN(ctx)
+    if (!out) return fail(eng, DMRG_EINVAL, "sweep_stats: null output");
+    out->seconds_environments = eng.t_env; out->seconds_restore = eng.t_restore; out->seconds_regrow = eng.t_regrow;
+    out->seconds_spill_wait = eng.t_spill_wait; out->seconds_maps = eng.t_plan; out->seconds_davidson = eng.t_davidson;
+    out->seconds_matvec = eng.t_matvec; out->seconds_split = eng.t_split; out->seconds_renormalise = eng.t_grow;
+    out->bytes_spilled = eng.spill_bytes; out->bytes_restored = eng.restore_bytes;
+    out->peak_device_bytes = eng.env_peak_bytes; out->host_pool_bytes = eng.host_pool.bytes;
+    out->est_stack_bytes = eng.env_est_total; out->est_max_block_bytes = eng.env_est_max;
+    out->env_stride = eng.env_stride; out->host_spill = eng.env_spill ? 1 : 0;
+    return DMRG_OK;
+    API_END
+}
+
 int dmrg_rdm12(dmrg_ctx* ctx, double* gamma, double* Gamma, int where, void* cuda_stream) {
     API_BEGIN(ctx)
-    (void)cuda_stream;
     if (!eng.have_mps) return fail(eng, DMRG_ESTATE, "rdm12: import an MPS first");
     if (!gamma) return fail(eng, DMRG_EINVAL, "rdm12: null gamma");
     const size_t k = (size_t)eng.k;
     if (where == DMRG_HOST) {
         rdm12(eng, gamma, Gamma);
     } else if (where == DMRG_DEVICE) {
+        // the pass runs on the library stream and ends synchronised; the results are then written to the caller's
+        // buffers on the caller's stream (ordered after its pending work on them), and the call returns when they are there
+        cudaStream_t cs = (cudaStream_t)cuda_stream;
         std::vector<double> g(k * k), G(Gamma ? k * k * k * k : 0);
         rdm12(eng, g.data(), Gamma ? G.data() : nullptr);
-        cuda_check(cudaMemcpy(gamma, g.data(), g.size() * 8, cudaMemcpyHostToDevice), "gamma upload");
-        if (Gamma) cuda_check(cudaMemcpy(Gamma, G.data(), G.size() * 8, cudaMemcpyHostToDevice), "Gamma upload");
+        cuda_check(cudaMemcpyAsync(gamma, g.data(), g.size() * 8, cudaMemcpyHostToDevice, cs), "gamma upload");
+        if (Gamma) cuda_check(cudaMemcpyAsync(Gamma, G.data(), G.size() * 8, cudaMemcpyHostToDevice, cs), "Gamma upload");
+        cuda_check(cudaStreamSynchronize(cs), "rdm12 upload");
     } else return fail(eng, DMRG_EINVAL, "rdm12: bad `where`");
     return DMRG_OK;
     API_END
@@ -423,7 +462,6 @@ int dmrg_grouped_gemm(int ntasks, const int64_t* c_ptr, const int32_t* ldc, cons
     try {
         Engine tmp;                                            // only the stream and the launch counter are used
         tmp.stream = (cudaStream_t)cuda_stream;
-        { const char* g = std::getenv("DMRG_B200_GENERIC_GEMM"); tmp.force_generic_gemm = g && g[0] == '1'; }
         GemmBatch b;
         for (int t = 0; t < ntasks; ++t) {
             if (seg_begin[t] < 0 || seg_count[t] < 0 || seg_begin[t] + seg_count[t] > nsegs) return DMRG_EINVAL;

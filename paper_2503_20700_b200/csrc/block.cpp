@@ -227,8 +227,91 @@ double run_once_ms(GemmBatch& b, Engine& eng) {
 Block::Block(char side_, int b_, int k_, const Basis& basis_, char mode_)
     : side(side_), b(b_), k(k_), mode(mode_), basis(basis_) {}
 Block::~Block() {
-    for (void* p : allocs) dev_free(p);
+    if (spill_done) { cudaEventSynchronize(spill_done); cudaEventDestroy(spill_done); }
+    for (BlockAlloc& a : allocs) {
+        if (a.dev) dev_free(a.dev);
+        if (a.host && pool) pool->put(a.host);
+    }
     for (void* p : temp_allocs) dev_free(p);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// pinned host pool and spill / restore of a block's storage
+// ---------------------------------------------------------------------------------------------------------------
+double* HostPool::get(size_t doubles) {
+    int best = -1;
+    for (size_t j = 0; j < regions.size(); ++j)              // best fit among free regions that are not wastefully large
+        if (!regions[j].used && regions[j].doubles >= doubles && regions[j].doubles <= doubles + doubles / 2 + 1024 &&
+            (best < 0 || regions[j].doubles < regions[best].doubles)) best = (int)j;
+    if (best >= 0) { regions[best].used = true; return regions[best].p; }
+    void* p = nullptr;
+    const cudaError_t e = cudaHostAlloc(&p, std::max<size_t>(doubles, 1) * sizeof(double), cudaHostAllocDefault);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        for (size_t j = 0; j < regions.size();)               // give back the free regions and retry once
+            if (!regions[j].used) { cudaFreeHost(regions[j].p); bytes -= (int64_t)regions[j].doubles * 8; regions.erase(regions.begin() + j); }
+            else ++j;
+        if (cudaHostAlloc(&p, std::max<size_t>(doubles, 1) * sizeof(double), cudaHostAllocDefault) != cudaSuccess) {
+            cudaGetLastError();
+            throw Error(-3, "pinned host memory exhausted while spilling an environment block");
+        }
+    }
+    regions.push_back({(double*)p, doubles, true});
+    bytes += (int64_t)doubles * 8;
+    return (double*)p;
+}
+void HostPool::put(double* p) {
+    for (Region& r : regions) if (r.p == p) { r.used = false; return; }
+}
+void HostPool::clear() {
+    for (Region& r : regions) cudaFreeHost(r.p);
+    regions.clear();
+    bytes = 0;
+}
+
+void Block::spill(HostPool& hp, cudaStream_t copy_stream) {
+    if (spilled) return;
+    if (!temp_allocs.empty()) throw std::logic_error("Block::spill: temporaries alive");
+    pool = &hp;
+    for (BlockAlloc& a : allocs) {
+        if (!a.dev) continue;
+        a.host = hp.get(a.doubles);
+        cuda_check(cudaMemcpyAsync(a.host, a.dev, a.doubles * sizeof(double), cudaMemcpyDeviceToHost, copy_stream), "spill");
+    }
+    if (!spill_done) cuda_check(cudaEventCreateWithFlags(&spill_done, cudaEventDisableTiming), "event");
+    cuda_check(cudaEventRecord(spill_done, copy_stream), "event record");
+    spilled = true;
+}
+void Block::finish_spill() {
+    if (!spilled) return;
+    if (spill_done) cuda_check(cudaEventSynchronize(spill_done), "spill wait");
+    for (BlockAlloc& a : allocs)
+        if (a.dev && a.host) { dev_free(a.dev); a.dev = nullptr; }
+}
+void Block::restore(cudaStream_t st) {
+    if (!spilled) return;
+    if (spill_done) cuda_check(cudaEventSynchronize(spill_done), "spill wait");
+    for (BlockAlloc& a : allocs) {
+        if (!a.host) continue;
+        if (!a.dev) {
+            a.dev = (double*)dev_alloc(a.doubles * sizeof(double));
+            cuda_check(cudaMemcpyAsync(a.dev, a.host, a.doubles * sizeof(double), cudaMemcpyHostToDevice, st), "restore");
+        }
+    }
+    cuda_check(cudaStreamSynchronize(st), "restore");
+    for (BlockAlloc& a : allocs)
+        if (a.host) { pool->put(a.host); a.host = nullptr; }
+    for (Stack& stk : stacks) {                                // device addresses changed: re-derive every pointer
+        if (stk.alloc < 0) continue;
+        stk.base = allocs[stk.alloc].dev ? allocs[stk.alloc].dev + stk.alloc_off : nullptr;
+        const int64_t ld = classes[stk.cls].ld;
+        for (size_t r = 0; r < stk.members.size(); ++r) {
+            auto it = ops.find(stk.members[r].key());
+            if (it != ops.end() && it->second.stack == (int)(&stk - stacks.data()))
+                it->second.ptr = stk.base ? stk.base + (int64_t)r * ld : nullptr;
+        }
+    }
+    spilled = false;
 }
 std::vector<int> Block::inside() const {
     std::vector<int> v;
@@ -295,15 +378,19 @@ void Block::allocate(const std::vector<Label>& labels, bool temp) {
     }
     int64_t total = 0;
     for (size_t s = first; s < stacks.size(); ++s) total += (int64_t)stacks[s].members.size() * classes[stacks[s].cls].ld;
+    if (spilled) throw std::logic_error("Block::allocate on a spilled block");
     double* base = (double*)dev_alloc((size_t)total * sizeof(double));
+    int alloc_idx = -1;
     if (base) {
-        (temp ? temp_allocs : allocs).push_back(base);
+        if (temp) temp_allocs.push_back(base);
+        else { BlockAlloc a; a.dev = base; a.doubles = (size_t)total; allocs.push_back(a); alloc_idx = (int)allocs.size() - 1; }
         cuda_check(cudaMemset(base, 0, (size_t)total * sizeof(double)), "memset");   // padding stays finite
     }
-    bytes_ += total * 8;
+    if (!temp) bytes_ += total * 8;
     int64_t off = 0;
     for (size_t s = first; s < stacks.size(); ++s) {
         Stack& st = stacks[s];
+        st.alloc = alloc_idx; st.alloc_off = off;
         st.base = base ? base + off : nullptr;
         const int64_t ld = classes[st.cls].ld;
         for (size_t r = 0; r < st.members.size(); ++r) ops[st.members[r].key()].ptr = st.base ? st.base + (int64_t)r * ld : nullptr;

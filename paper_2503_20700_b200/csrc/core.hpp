@@ -106,7 +106,21 @@ struct Stack {                                    // operators of one (kind, cla
     int kind, cls;
     double* base = nullptr;
     std::vector<Label> members;
+    int alloc = -1;                               // index into Block::allocs (-1: temporary storage)
+    int64_t alloc_off = 0;                        // offset of the stack inside that allocation (doubles)
 };
+// Pinned host memory for spilled environment blocks (SURVEY.md 7 hard part 5): regions are reused across passes and
+// sweeps because pinning is slow (seconds per 10 GB); freed with the context.
+struct HostPool {
+    struct Region { double* p; size_t doubles; bool used; };
+    std::vector<Region> regions;
+    int64_t bytes = 0;
+    double* get(size_t doubles);
+    void put(double* p);
+    void clear();
+    ~HostPool() { clear(); }
+};
+struct BlockAlloc { double* dev = nullptr; size_t doubles = 0; double* host = nullptr; };
 struct OpRef { int cls = -1; double* ptr = nullptr; int stack = -1, row = -1; };
 
 struct Block {
@@ -117,8 +131,11 @@ struct Block {
     std::vector<OpClass> classes;
     std::vector<Stack> stacks;
     std::unordered_map<uint32_t, OpRef> ops;
-    std::vector<void*> allocs;                    // persistent device allocations
+    std::vector<BlockAlloc> allocs;               // persistent storage: on the device, or spilled to pinned host memory
     std::vector<void*> temp_allocs;               // temporaries of make_temps
+    bool spilled = false;                         // storage lives in allocs[].host; restore() before use
+    cudaEvent_t spill_done = nullptr;             // device copies may be freed once this event has completed
+    HostPool* pool = nullptr;
     std::vector<uint32_t> temp_keys;
     Block(char side, int b, int k, const Basis& basis, char mode);
     ~Block();
@@ -135,6 +152,11 @@ struct Block {
     void drop_kind(int kind);                     // forget operators of a kind (storage is released with the block)
     int64_t bytes() const;
     int64_t bytes_ = 0;
+    // environment-stack memory path: asynchronous device -> pinned host copy on `copy_stream`; finish_spill() waits for
+    // it and frees the device storage; restore() brings the block back and re-derives every operator pointer
+    void spill(HostPool& pool, cudaStream_t copy_stream);
+    void finish_spill();
+    void restore(cudaStream_t st);
 };
 
 // a dense block of an operator as the GEMM kernel sees it
@@ -198,6 +220,14 @@ struct Options {
     double sv_floor = 1e-10, cluster_rel_gap = 1e-6;
     int device_id = 0;
     int64_t workspace_bytes = 0;
+    int64_t hbm_budget_bytes = 0;                 // device bytes the environment stack of a sweep may hold (0 = automatic)
+    int64_t host_budget_bytes = 0;                // pinned host bytes for spilled checkpoints (0 = automatic: 96 GiB)
+    int host_spill = 0;                           // 1: environment checkpoints may live in pinned host memory
+    int env_stride = 0;                           // checkpoint spacing of the environment stack (0 = automatic, 1 = keep all)
+    double dbss_eps = 0.0;                        // > 0: dynamic block state selection, truncation error target per bond
+    int dbss_dmin = 0;                            // DBSS lower bound on the kept states
+    int split_k = 0;                              // split-K parts of phase 2 of H_eff psi (0 = automatic)
+    int svd_qr = 0;                               // 1: QR-iteration SVD (gesvd) instead of one-sided Jacobi (gesvdj)
 };
 struct BondRecord {
     int bond, forward;
@@ -224,14 +254,31 @@ struct Engine {
     double t_plan = 0, t_davidson = 0, t_split = 0, t_grow = 0, t_matvec = 0;   // phase seconds of the last sweep
     double rdm_stream_ms = 0;                     // device time of the operator-streaming kernels (E = Stack M^T) alone
     bool keep_env_stack = true;
+    // environment-stack memory path of dmrg_sweep (row "m"): checkpoints every env_stride bonds, the blocks between two
+    // checkpoints are recomputed when a pass enters that segment; checkpoints optionally spilled to pinned host memory
+    int env_stride = 1;
+    bool env_spill = false;
+    HostPool host_pool;
+    cudaStream_t copy_stream = nullptr;
+    std::vector<Block*> pending_spills;
+    double t_spill_wait = 0, t_restore = 0, t_regrow = 0, spill_bytes = 0, restore_bytes = 0, t_env = 0;
+    int env_D = 0;
+    int64_t env_peak_bytes = 0, env_est_total = 0, env_est_max = 0;
+    void plan_env_policy(int D);                  // choose env_stride / env_spill from the options and the memory estimate
+    void finish_spills();
+    Block& need_left(int b);                      // device-resident L_b (restored or regrown from the nearest checkpoint)
+    Block& need_right(int b);
+    void retire_left(int b);                      // L_b has produced L_{b+1}: keep as checkpoint (spill) or erase
+    void retire_right(int b);
+    void build_right_stack();                     // R_k .. R_2 under the policy (start of the first sweep)
     bool sweep_ready = false;                     // environments consistent with the sweep position
-    bool host_maps = false;                       // DMRG_B200_HOST_MAPS=1: build the H_eff block maps on the host (A/B testing)
+    bool host_maps = false;                       // dmrg_options.host_maps: build the H_eff block maps on the host (A/B testing)
     bool trace = false;                           // DMRG_B200_TRACE=1: print every grouped-GEMM launch's device time
-    bool force_generic_gemm = false;              // DMRG_B200_GENERIC_GEMM=1: always the cp.async kernel (A/B testing)
+    bool force_generic_gemm = false;              // dmrg_options.generic_gemm: always the cp.async kernel (A/B testing)
     char mode_L(int b) const { return b <= bsw ? 'N' : 'C'; }
     char mode_R(int b) const { return b >= bsw + 3 ? 'N' : 'C'; }
     int64_t t_capacity() const;                   // doubles available for intermediates
-    void invalidate() { plan.reset(); L.clear(); R.clear(); sweep_ready = false; }   // the plan owns temporaries on a block
+    void invalidate() { plan.reset(); pending_spills.clear(); L.clear(); R.clear(); sweep_ready = false; }   // the plan owns temporaries on a block
     void ensure_left(int i);                      // L_0 .. L_i present
     void ensure_right(int j);                     // R_k .. R_j present
     void prepare_bond(int i);

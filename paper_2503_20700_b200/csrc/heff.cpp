@@ -222,7 +222,7 @@ static void build_maps_device(HeffPlan& p, const std::vector<NTerm>& terms, Bloc
         // the tiles of one output block closer together in time, which helps the L2 hit rate of their shared panels
         const int64_t target = (int64_t)sms * 3 * 64;
         if (base_tiles > 0) S = (int)std::min<int64_t>(16, std::max<int64_t>(1, (target + base_tiles - 1) / base_tiles));
-        if (const char* g = std::getenv("DMRG_B200_SPLITK")) S = std::max(1, std::min(16, std::atoi(g)));
+        if (eng.opt.split_k > 0) S = std::min(16, eng.opt.split_k);
     }
     p.split = S;
     if (S > 1) p.ypart.alloc((size_t)(S - 1) * (size_t)std::max<int64_t>(p.nnz, 1));

@@ -83,7 +83,7 @@ void launch_stack_dots(const double* S, int64_t lds, int nrows, const double* M,
 // ---- dense SVD of a row-major [m x n] matrix (cuSOLVER gesvd; library call) -----------------------
 // U [m x r], S [r], Vt [r x n] row-major, r = min(m, n); A is destroyed.  work: opaque per-engine handle.
 struct SvdWork;
-SvdWork* svd_create(cudaStream_t st);
+SvdWork* svd_create(cudaStream_t st, bool jacobi);   // jacobi: gesvdj (gesvd fallback), else gesvd
 void svd_destroy(SvdWork* w);
 void svd_rowmajor(SvdWork* w, double* A, int m, int n, double* U, double* S, double* Vt, cudaStream_t st);
 

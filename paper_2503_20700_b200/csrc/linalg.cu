@@ -32,7 +32,7 @@ static void cu_check(cudaError_t e, const char* what) {
     if (e != cudaSuccess) throw std::runtime_error(std::string(what) + ": " + cudaGetErrorString(e));
 }
 
-SvdWork* svd_create(cudaStream_t st) {
+SvdWork* svd_create(cudaStream_t st, bool jacobi) {
     SvdWork* w = new SvdWork();
     cs_check(cusolverDnCreate(&w->h), "cusolverDnCreate");
     cs_check(cusolverDnSetStream(w->h, st), "cusolverDnSetStream");
@@ -40,7 +40,7 @@ SvdWork* svd_create(cudaStream_t st) {
     cs_check(cusolverDnCreateGesvdjInfo(&w->jparams), "CreateGesvdjInfo");
     cs_check(cusolverDnXgesvdjSetSortEig(w->jparams, 1), "gesvdj sort");
     cs_check(cusolverDnXgesvdjSetMaxSweeps(w->jparams, 100), "gesvdj sweeps");
-    { const char* g = std::getenv("DMRG_B200_SVD_QR"); w->use_jacobi = !(g && g[0] == '1'); }
+    w->use_jacobi = jacobi;
     return w;
 }
 void svd_destroy(SvdWork* w) {

@@ -296,6 +296,148 @@ void split_theta(MPS& mps, int i, const HeffPlan& p, const double* theta, int D,
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// Environment-stack memory path (SURVEY.md 7 hard part 5; BASELINE configs 4 and 5: "block-sparse operator storage
+// sized to fit 180 GB HBM").  A pass consumes the blocks of one side in the order the previous pass produced them
+// reversed, so only every env_stride-th block (a checkpoint) is kept; when the pass enters the segment between two
+// checkpoints, its blocks are recomputed from the checkpoint with the unchanged site tensors (one extra blocking step
+// per block and pass - renormalisation is a few percent of a sweep).  Checkpoints may additionally be spilled to
+// pinned host memory with an asynchronous copy on a separate stream and fetched back when their segment is entered.
+// ---------------------------------------------------------------------------------------------------------------
+static double wall() { return std::chrono::duration<double>(std::chrono::steady_clock::now().time_since_epoch()).count(); }
+
+static int64_t g_device_bytes_env(const Engine& eng) {         // device bytes held by environment blocks right now
+    int64_t b = 0;
+    for (const auto& kv : eng.L) if (!kv.second->spilled) b += kv.second->bytes();
+    for (const auto& kv : eng.R) if (!kv.second->spilled) b += kv.second->bytes();
+    return b;
+}
+static void erase_block(Engine& eng, std::map<int, std::unique_ptr<Block>>& side, std::map<int, std::unique_ptr<Block>>::iterator& it) {
+    for (size_t j = 0; j < eng.pending_spills.size(); ++j)
+        if (eng.pending_spills[j] == it->second.get()) { eng.pending_spills.erase(eng.pending_spills.begin() + j); break; }
+    it = side.erase(it);
+}
+
+void Engine::plan_env_policy(int D) {
+    // estimate of every left block's bytes at bond dimension D from the current sector structure
+    std::vector<double> est(k + 1, 0.0);
+    double total = 0.0, bmax = 0.0;
+    for (int b = 0; b <= k; ++b) {
+        double sumsq = 0.0, dcur = 0.0;
+        for (const Sector& q : mps.bonds[b]) { sumsq += (double)q.d * q.d; dcur += q.d; }
+        // exact Schmidt bound of the bond, evaluated in log space (4^b overflows a double only beyond k ~ 500)
+        const double lg4 = std::log2(4.0) * std::min(b, k - b);
+        const double cap = lg4 < 40 ? std::min((double)D, std::pow(2.0, lg4)) : (double)D;
+        if (dcur < cap && dcur > 0) sumsq *= (cap / dcur) * (cap / dcur);
+        const double nin = 2.0 * std::min(b, k - b), nall = 2.0 * k;
+        const double nops = nin * (nin - 1) / 2 + nin * nin + nall + 1;
+        est[b] = 8.0 * nops * sumsq;
+        total += est[b];
+        bmax = std::max(bmax, est[b]);
+    }
+    env_est_total = (int64_t)total; env_est_max = (int64_t)bmax;
+    size_t free_b = 0, total_b = 0;
+    cuda_check(cudaMemGetInfo(&free_b, &total_b), "cudaMemGetInfo");
+    // what is free now also has to hold the intermediates of H_eff psi and of the blocking step, the Davidson subspace
+    // and the block being grown: the stack gets 55 % of it unless the caller fixes a budget
+    const double budget = opt.hbm_budget_bytes > 0 ? (double)opt.hbm_budget_bytes : 0.55 * ((double)free_b + (double)g_device_bytes_env(*this));
+    const double host_budget = opt.host_budget_bytes > 0 ? (double)opt.host_budget_bytes : 96.0 * (double)(1ull << 30);
+    env_spill = false;
+    if (opt.env_stride > 0) { env_stride = opt.env_stride; env_spill = opt.host_spill != 0; return; }
+    if (total <= budget) { env_stride = 1; return; }
+    if (opt.host_spill) {
+        // checkpoints on the host, the segment being consumed (stride blocks) plus the block being produced on the device
+        int s = 1;
+        while (s < k && total / s > host_budget) ++s;
+        if ((s + 1) * bmax > budget) throw Error(-3, "environment stack: one segment between host checkpoints exceeds the device budget");
+        while (s + 1 < k && (s + 2) * bmax <= 0.5 * budget) ++s;      // fewer, larger segments: fewer host round trips
+        env_stride = s; env_spill = true;
+        return;
+    }
+    int best = 0;
+    double best_need = 0.0;
+    for (int s = 1; s <= k; ++s) {
+        const double need = total / s + (s + 1) * bmax;
+        if (!best || need < best_need) { best = s; best_need = need; }
+    }
+    if (best_need > budget) throw Error(-3, "environment stack does not fit the device even with recomputation: set host_spill = 1");
+    int s = 1;
+    while (total / s + (s + 1) * bmax > budget) ++s;                  // smallest stride that fits: least recomputation
+    env_stride = s;
+}
+
+void Engine::finish_spills() {
+    const double t0 = wall();
+    for (Block* b : pending_spills) b->finish_spill();
+    pending_spills.clear();
+    t_spill_wait += wall() - t0;
+}
+
+static bool is_checkpoint(const Engine& eng, int b) { return b == 0 || b == eng.k || b % eng.env_stride == 0; }
+
+void Engine::retire_left(int b) {
+    auto it = L.find(b);
+    if (it == L.end() || b == 0) return;
+    if (!is_checkpoint(*this, b)) { erase_block(*this, L, it); return; }
+    if (env_spill && !it->second->spilled) {
+        spill_bytes += (double)it->second->bytes();
+        it->second->spill(host_pool, copy_stream);
+        pending_spills.push_back(it->second.get());
+    }
+}
+void Engine::retire_right(int b) {
+    auto it = R.find(b);
+    if (it == R.end() || b == k) return;
+    if (!is_checkpoint(*this, b)) { erase_block(*this, R, it); return; }
+    if (env_spill && !it->second->spilled) {
+        spill_bytes += (double)it->second->bytes();
+        it->second->spill(host_pool, copy_stream);
+        pending_spills.push_back(it->second.get());
+    }
+}
+static void make_resident(Engine& eng, Block& blk) {
+    if (!blk.spilled) return;
+    const double t0 = wall();
+    for (size_t j = 0; j < eng.pending_spills.size(); ++j)
+        if (eng.pending_spills[j] == &blk) { eng.pending_spills.erase(eng.pending_spills.begin() + j); break; }
+    eng.restore_bytes += (double)blk.bytes();
+    blk.restore(eng.stream);
+    eng.t_restore += wall() - t0;
+}
+Block& Engine::need_left(int b) {
+    auto it = L.find(b);
+    if (it != L.end()) { make_resident(*this, *it->second); return *it->second; }
+    int c = b;
+    while (c > 0 && L.find(c) == L.end()) --c;                        // nearest checkpoint below
+    if (L.find(c) == L.end()) L[0] = empty_block('L', k, mps);
+    make_resident(*this, *L.at(c));
+    const double t0 = wall();
+    for (int j = c; j < b; ++j) L[j + 1] = grow(*L.at(j), ham, mps, mode_L(j + 1), *this);
+    t_regrow += wall() - t0;
+    return *L.at(b);
+}
+Block& Engine::need_right(int b) {
+    auto it = R.find(b);
+    if (it != R.end()) { make_resident(*this, *it->second); return *it->second; }
+    int c = b;
+    while (c < k && R.find(c) == R.end()) ++c;
+    if (R.find(c) == R.end()) R[k] = empty_block('R', k, mps);
+    make_resident(*this, *R.at(c));
+    const double t0 = wall();
+    for (int j = c; j > b; --j) R[j - 1] = grow(*R.at(j), ham, mps, mode_R(j - 1), *this);
+    t_regrow += wall() - t0;
+    return *R.at(b);
+}
+void Engine::build_right_stack() {
+    if (R.find(k) == R.end()) R[k] = empty_block('R', k, mps);
+    for (int b = k; b > 2; --b) {
+        finish_spills();
+        R[b - 1] = grow(*R.at(b), ham, mps, mode_R(b - 1), *this);
+        retire_right(b);
+    }
+}
+static void track_peak(Engine& eng) { eng.env_peak_bytes = std::max(eng.env_peak_bytes, g_device_bytes); }
+
+// ---------------------------------------------------------------------------------------------------------------
 // one sweep: forward pass over bonds 0..k-2, backward pass k-2..0 (reading S12)
 // ---------------------------------------------------------------------------------------------------------------
 static BondRecord optimise(Engine& eng, int i, int D, bool forward) {
@@ -303,7 +445,11 @@ static BondRecord optimise(Engine& eng, int i, int D, bool forward) {
     auto secs = [](clk::time_point a, clk::time_point b) { return std::chrono::duration<double>(b - a).count(); };
     const auto t0 = clk::now();
     eng.plan.reset();
-    eng.plan = build_heff(eng.ham, *eng.L.at(i), *eng.R.at(i + 2), i, eng);
+    eng.finish_spills();                                       // device copies of blocks spilled during the previous step
+    Block& LB = eng.need_left(i);
+    Block& RB = eng.need_right(i + 2);
+    const auto t0b = clk::now();
+    eng.plan = build_heff(eng.ham, LB, RB, i, eng);
     HeffPlan& p = *eng.plan;
     const auto t1 = clk::now();
     DevVec<double> theta;
@@ -318,11 +464,27 @@ static BondRecord optimise(Engine& eng, int i, int D, bool forward) {
     split_theta(eng.mps, i, p, theta.p, D, forward, eng, rec.trunc_err, rec.kept, rec.nsectors);
     const auto t3 = clk::now();
     eng.plan.reset();                                          // releases the temporaries before the block grows
-    if (forward) eng.L[i + 1] = grow(*eng.L.at(i), eng.ham, eng.mps, eng.mode_L(i + 1), eng);
-    else         eng.R[i + 1] = grow(*eng.R.at(i + 2), eng.ham, eng.mps, eng.mode_R(i + 1), eng);
+    track_peak(eng);
+    if (forward) {
+        // blocks of the right stack up to bond i+2 are consumed (the backward pass rebuilds them); L_i has produced
+        // L_{i+1} and stays only as a checkpoint
+        for (auto it = eng.R.begin(); it != eng.R.end();)
+            if (it->first <= i + 2 && it->first < eng.k) erase_block(eng, eng.R, it); else ++it;
+        eng.L[i + 1] = grow(LB, eng.ham, eng.mps, eng.mode_L(i + 1), eng);
+        if (i < eng.k - 2) eng.retire_left(i);                 // the backward pass starts at this bond: keep L_{k-2}
+    } else {
+        for (auto it = eng.L.begin(); it != eng.L.end();)      // L_i is consumed, every L_b with b > i is stale
+            if (it->first >= i && it->first > 0) erase_block(eng, eng.L, it); else ++it;
+        if (i > 0) {                                           // R_1 is never used; the next forward pass starts from R_2
+            eng.R[i + 1] = grow(RB, eng.ham, eng.mps, eng.mode_R(i + 1), eng);
+            eng.retire_right(i + 2);
+        }
+    }
+    track_peak(eng);
     const auto t4 = clk::now();
     rec.seconds = secs(t0, t4);
-    eng.t_plan += secs(t0, t1); eng.t_davidson += secs(t1, t2); eng.t_split += secs(t2, t3); eng.t_grow += secs(t3, t4);
+    eng.t_env += secs(t0, t0b);
+    eng.t_plan += secs(t0b, t1); eng.t_davidson += secs(t1, t2); eng.t_split += secs(t2, t3); eng.t_grow += secs(t3, t4);
     eng.t_matvec += dr.seconds_matvec;
     return rec;
 }
@@ -330,21 +492,31 @@ static BondRecord optimise(Engine& eng, int i, int D, bool forward) {
 int sweep(Engine& eng, int D, std::vector<BondRecord>& recs, double& seconds) {
     const auto t0 = std::chrono::steady_clock::now();
     const int k = eng.k;
-    if (!eng.sweep_ready) {
-        eng.invalidate();
-        eng.keep_env_stack = true;
-        eng.L[0] = empty_block('L', k, eng.mps);
-        eng.ensure_right(2);
-        eng.sweep_ready = true;
+    eng.t_plan = eng.t_davidson = eng.t_split = eng.t_grow = eng.t_matvec = eng.t_env = 0.0;
+    eng.t_spill_wait = eng.t_restore = eng.t_regrow = eng.spill_bytes = eng.restore_bytes = 0.0;
+    eng.env_peak_bytes = 0;
+    if (!eng.sweep_ready || D != eng.env_D) {
+        const bool rebuild = !eng.sweep_ready;
+        if (rebuild) eng.invalidate();
+        eng.plan_env_policy(D);
+        eng.env_D = D;
+        if (rebuild) {
+            eng.keep_env_stack = true;
+            eng.L[0] = empty_block('L', k, eng.mps);
+            const double tb = wall();
+            eng.build_right_stack();
+            eng.t_env += wall() - tb;
+            eng.sweep_ready = true;
+        }
     }
     recs.clear();
-    eng.t_plan = eng.t_davidson = eng.t_split = eng.t_grow = eng.t_matvec = 0.0;
     for (int i = 0; i <= k - 2; ++i) recs.push_back(optimise(eng, i, D, true));
     for (int i = k - 2; i >= 0; --i) recs.push_back(optimise(eng, i, D, false));
     seconds = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
     if (eng.trace || std::getenv("DMRG_B200_TIMERS"))
-        std::fprintf(stderr, "[dmrg trace] sweep D=%d: %.2f s = plan (block maps) %.2f + davidson %.2f (matvec %.2f) + svd/split %.2f + renormalise %.2f\n",
-                     D, seconds, eng.t_plan, eng.t_davidson, eng.t_matvec, eng.t_split, eng.t_grow);
+        std::fprintf(stderr, "[dmrg trace] sweep D=%d: %.2f s = environments (restore %.2f, regrow %.2f, spill wait %.2f) %.2f + plan (block maps) %.2f + davidson %.2f (matvec %.2f) + svd/split %.2f + renormalise %.2f; stride %d spill %d peak %.1f GB\n",
+                     D, seconds, eng.t_restore, eng.t_regrow, eng.t_spill_wait, eng.t_env, eng.t_plan, eng.t_davidson, eng.t_matvec, eng.t_split, eng.t_grow,
+                     eng.env_stride, (int)eng.env_spill, eng.env_peak_bytes / 1e9);
     int warnings = 0;
     for (const BondRecord& r : recs) if (!r.converged) ++warnings;
     return warnings;

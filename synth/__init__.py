@@ -6,4 +6,4 @@ Recipes: BASELINE.json configs[0..4]; readings S6-S10, S15, S23 of SURVEY.md sec
 """
 from .hamiltonians import (hex_graph, flake_centres, row_centres, ppp_integrals, rotate_orbitals, fiedler_order,
                            permute_orbitals, fes_like, make_config, random_dense, CONFIG_SEED)
-from .mps import (random_mps, bond_sector_plan, full_sector_dims, mps_to_blob_arrays, blob_arrays_to_mps, SITE_Q)
+from .mps import (random_mps, dual_gauge_mps, mixed_gauge, bond_sector_plan, full_sector_dims, mps_to_blob_arrays, blob_arrays_to_mps, SITE_Q)

@@ -145,6 +145,24 @@ def random_mps(k, n_elec, two_sz, D, seed, gauge="R", plan=None):
     return dict(k=k, n_elec=n_elec, two_sz=two_sz, bonds=bonds, tensors=tensors, gauge=gl)
 
 
+def dual_gauge_mps(k, n_elec, two_sz, D, seed):
+    """A left-orthonormal MPS A (seed) and a right-orthonormal MPS B (seed + 1) on ONE sector plan: H_eff at any
+    two-site bond i is defined by A on sites < i and B on sites > i + 1, so one pair serves every bond."""
+    plan = bond_sector_plan(k, n_elec, two_sz, D)
+    A = random_mps(k, n_elec, two_sz, D, seed=seed, gauge="L", plan=plan)
+    B = random_mps(k, n_elec, two_sz, D, seed=seed + 1, gauge="R", plan=plan)
+    return A, B
+
+
+def mixed_gauge(A, B, i):
+    """Sites < i from A (left-orthonormal), sites >= i from B (right-orthonormal); same bonds."""
+    k = A["k"]
+    assert A["bonds"] == B["bonds"]
+    return dict(k=k, n_elec=A["n_elec"], two_sz=A["two_sz"], bonds=A["bonds"],
+                tensors=[A["tensors"][p] if p < i else B["tensors"][p] for p in range(k)],
+                gauge=["L" if p < i else "R" for p in range(k)])
+
+
 def mps_to_blob_arrays(mps):
     """Flatten to the C-ABI blob: (bond_ptr[k+2], sec_N, sec_S2, sec_dim, blk_ptr[k+1], blk_l, blk_s, blk_off, data,
     gauge bytes).  Blocks of a site are ordered by (l_idx, s); offsets are in doubles into `data`."""

@@ -1,22 +1,45 @@
-"""Writes the stored expected values under tests/golden/ by calling ONLY oracle/ (tier-1 brute-force full CI) on the
-seeded generators of synth/.  Nothing here imports the CUDA package.  Run: python tests/golden/make_golden.py
+"""Writes the stored expected values under tests/golden/ by calling ONLY oracle/ on the seeded generators of synth/.
+Nothing here imports the CUDA package.  Each file records the command that wrote it and how long the oracle took.
 
-config1_fci.txt - BASELINE.json configs[0] (PPP naphthalene CAS(10,10), 2Sz = 0, FCI dimension 63504, readings S6-S9
-of DESIGN.md): E_core, E_el(FCI), E_total, Tr gamma and the natural occupations of the FCI 1-RDM (Eq. 9).
-The total energy is seed independent (invariant under the exp(kappa) rotation) and agrees with the survey's
-independent probe value -0.8822829988 Eh."""
+  python tests/golden/make_golden.py fci
+      config1_fci.txt - BASELINE.json configs[0] (PPP naphthalene CAS(10,10), 2Sz = 0, FCI dimension 63504, readings
+      S6-S9 of DESIGN.md): E_core, E_el(FCI), E_total, Tr gamma and the natural occupations of the FCI 1-RDM
+      (Eq. 9) from oracle/fci.py.  The total energy is seed independent (invariant under the exp(kappa)
+      rotation) and agrees with the survey's independent probe value -0.8822829988 Eh.
+
+  python tests/golden/make_golden.py heff CFG D BOND [BOND ...]
+      heff_cfgC_DD.npz - y = H_eff x (y = P^T H P x, Eq. 1-5 and 122-130 Eq. 14-15; C2),
+      diag(H_eff) and the oracle's own GEMM-flop count at the listed two-site bonds of BASELINE config CFG at bond
+      dimension D, from oracle/dmrg.py (tier 2) on its own environments.  Inputs: the "dual gauge" pair of seeded MPS
+      (left-orthonormal A with seed s, right-orthonormal B with seed s + 1 on one sector plan, s = config seed + 2000)
+      and x = normalised N(0,1) vector from default_rng(1000 + bond) - tests/test_gpu_golden.py rebuilds the same
+      inputs for the CUDA library.  The plain Python oracle cannot reach the configs' own D (4096 / 2048) on k = 54 /
+      82 in bounded time; the files say which D it did reach and how long that took.
+
+  python tests/golden/make_golden.py sweep CFG D NSWEEPS [DINIT]
+      sweep_cfgC_DD.json - per-bond Davidson energies, kept bond dimension, sector count and truncation error of
+      NSWEEPS two-site sweeps (readings S12-S18, Davidson tolerance 1e-10 as in S13) from oracle.dmrg.SweepEngine on
+      random_mps(seed = config seed + 1000, gauge R, D = DINIT or D).
+
+  python tests/golden/make_golden.py rdm CFG D
+      rdm_cfgC_DD.npz - gamma and Gamma (Eq. 9-10, readings S2 / S20) of random_mps(seed = 900 + CFG,
+      gauge R) from oracle.dmrg.rdm12.
+"""
+import json
 import os
 import sys
+import time
 
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, os.path.dirname(os.path.dirname(HERE)))
+from oracle import dmrg as odmrg  # noqa: E402
 from oracle import fci  # noqa: E402
-from synth import make_config  # noqa: E402
+from synth import dual_gauge_mps, make_config, random_mps  # noqa: E402
 
 
-def main():
+def golden_fci():
     cfg = make_config(1)
     sp = fci.FCISpace(cfg["k"], cfg["n_elec"], 0)
     e, c = sp.ground_state(cfg["h"], cfg["eri"], tol=1e-12)
@@ -29,6 +52,87 @@ def main():
         f.write("e_total_fci %.10f\n" % (e + cfg["e_core"]))
         f.write("trace_gamma %.10f\n" % np.trace(g))
         f.write("natural_occupations " + " ".join("%.8f" % x for x in occ) + "\n")
+
+
+def golden_heff(cid, D, bonds):
+    cfg = make_config(cid)
+    A, B = dual_gauge_mps(cfg["k"], cfg["n_elec"], 0, D, cfg["seed"] + 2000)
+    ham = odmrg.Ham(cfg["h"], cfg["eri"])
+    t0 = time.time()
+    oL = odmrg.build_left(A, ham, max(bonds))
+    oR = odmrg.build_right(B, ham, min(bonds) + 2)
+    t_env = time.time() - t0
+    out = dict(bonds=np.array(bonds), D=D, config=cid, mps_seed=cfg["seed"] + 2000)
+    secs = {}
+    for i in bonds:
+        t0 = time.time()
+        H = odmrg.Heff(oL[i], oR[i + 2], ham, i)
+        x = np.random.default_rng(1000 + i).normal(size=H.nnz)
+        x /= np.linalg.norm(x)
+        out["y_%d" % i] = H.apply(x)
+        out["diag_%d" % i] = H.diagonal()
+        out["nnz_%d" % i] = H.nnz
+        out["nterms_%d" % i] = len(H.terms)
+        out["gemm_flops_%d" % i] = H.gemm_flops()
+        out["layout_%d" % i] = np.array([b[:6] for b in H.layout], dtype=np.int64)
+        secs[i] = time.time() - t0
+        print("config %d D=%d bond %d: nnz=%d, %.0f s" % (cid, D, i, H.nnz, secs[i]), flush=True)
+    out["note"] = ("written by `python tests/golden/make_golden.py heff %d %d %s` from oracle/dmrg.py; oracle time: "
+                   "environments %.0f s, per bond %s s on %d host cores" %
+                   (cid, D, " ".join(map(str, bonds)), t_env, {i: round(s) for i, s in secs.items()}, os.cpu_count()))
+    np.savez_compressed(os.path.join(HERE, "heff_cfg%d_D%d.npz" % (cid, D)), **out)
+    print(out["note"], flush=True)
+
+
+def golden_sweep(cid, D, nsweeps, Dinit):
+    cfg = make_config(cid)
+    k, n = cfg["k"], cfg["n_elec"]
+    mps = random_mps(k, n, 0, Dinit, seed=cfg["seed"] + 1000, gauge="R")
+    t0 = time.time()
+    eng = odmrg.SweepEngine(cfg["h"], cfg["eri"], mps, davidson_tol=1e-10)
+    sweeps = []
+    for s in range(nsweeps):
+        r = eng.sweep(D)
+        sweeps.append(r)
+        print("config %d D=%d sweep %d: E_last = %.12f (%.0f s)" % (cid, D, s, r["energy_last"], time.time() - t0), flush=True)
+    note = ("written by `python tests/golden/make_golden.py sweep %d %d %d %d` from oracle.dmrg.SweepEngine "
+            "(Davidson tol 1e-10); oracle time %.0f s on %d host cores" % (cid, D, nsweeps, Dinit, time.time() - t0, os.cpu_count()))
+    with open(os.path.join(HERE, "sweep_cfg%d_D%d.json" % (cid, D)), "w") as f:
+        json.dump(dict(note=note, config=cid, D=D, Dinit=Dinit, mps_seed=cfg["seed"] + 1000, davidson_tol=1e-10,
+                       sweeps=[dict(energy_last=r["energy_last"], energy_min=r["energy_min"],
+                                    bonds=[dict(bond=b["bond"], dir=b["dir"], energy=b["energy"], kept=b["kept"],
+                                                nsectors=b["nsectors"], trunc_err=b["trunc_err"], nnz=b["nnz"],
+                                                n_matvec=b["n_matvec"]) for b in r["bonds"]]) for r in sweeps]),
+                  f, indent=0)
+    print(note, flush=True)
+
+
+def golden_rdm(cid, D):
+    cfg = make_config(cid)
+    k, n = cfg["k"], cfg["n_elec"]
+    mps = random_mps(k, n, 0, D, seed=900 + cid, gauge="R")
+    t0 = time.time()
+    g, G = odmrg.rdm12(cfg["h"], cfg["eri"], mps, True)
+    note = ("written by `python tests/golden/make_golden.py rdm %d %d` from oracle.dmrg.rdm12; oracle time %.0f s on "
+            "%d host cores" % (cid, D, time.time() - t0, os.cpu_count()))
+    np.savez_compressed(os.path.join(HERE, "rdm_cfg%d_D%d.npz" % (cid, D)), gamma=g, Gamma=G, D=D, config=cid,
+                        mps_seed=900 + cid, note=note)
+    print(note, flush=True)
+
+
+def main():
+    what = sys.argv[1] if len(sys.argv) > 1 else "fci"
+    a = [int(x) for x in sys.argv[2:]]
+    if what == "fci":
+        golden_fci()
+    elif what == "heff":
+        golden_heff(a[0], a[1], a[2:])
+    elif what == "sweep":
+        golden_sweep(a[0], a[1], a[2], a[3] if len(a) > 3 else a[1])
+    elif what == "rdm":
+        golden_rdm(a[0], a[1])
+    else:
+        raise SystemExit(__doc__)
 
 
 if __name__ == "__main__":

@@ -1,0 +1,104 @@
+"""CUDA path vs stored oracle results (tests/golden/, written by tests/golden/make_golden.py from oracle/ alone) at
+sizes the plain Python oracle only reaches offline: H_eff psi and diag(H_eff) on the k = 54 (BASELINE config 4) and
+k = 82 (config 5) Hamiltonians - the 9 279 / 18 715-term lists with the N/C-mode switch on either side of the bond -,
+two-site sweeps of configs 2 and 3, and the 1-/2-RDMs of configs 2 and 3 at bond dimensions where operator classes
+have many right-hand sides and several K spans.  Inputs are rebuilt here from the same seeded generators (synth/).
+Tolerances (BASELINE.json north_star): H_eff psi rel. L2 <= 1e-11, RDM max-abs <= 1e-10, sweep energies <= 1e-8 Eh."""
+import glob
+import json
+import os
+
+import numpy as np
+import pytest
+
+from synth import dual_gauge_mps, make_config, mixed_gauge, mps_to_blob_arrays, random_mps
+
+pytestmark = pytest.mark.gpu
+GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+def _files(pattern):
+    return sorted(os.path.basename(f) for f in glob.glob(os.path.join(GOLD, pattern)))
+
+
+def test_golden_files_present():
+    """configs 4 and 5 must have an H_eff golden, configs 2 and 3 a sweep and an RDM golden."""
+    for c in (4, 5):
+        assert _files("heff_cfg%d_D*.npz" % c)
+    for c in (2, 3):
+        assert _files("sweep_cfg%d_D*.json" % c) and _files("rdm_cfg%d_D*.npz" % c)
+
+
+@pytest.mark.parametrize("name", _files("heff_cfg*_D*.npz"))
+def test_heff_vs_golden(lib, name):
+    z = np.load(os.path.join(GOLD, name), allow_pickle=False)
+    cid, D = int(z["config"]), int(z["D"])
+    cfg = make_config(cid)
+    k, n = cfg["k"], cfg["n_elec"]
+    A, B = dual_gauge_mps(k, n, 0, D, int(z["mps_seed"]))
+    ctx = lib.dmrg_create(k, n, 0, cfg["h"], cfg["eri"], keep_env_stack=0)
+    try:
+        for i in [int(b) for b in z["bonds"]]:
+            lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mixed_gauge(A, B, i)), k, n, 0)
+            lib.dmrg_prepare_bond(ctx, i)
+            nnz, lay = lib.dmrg_heff_layout(ctx, i)
+            assert nnz == int(z["nnz_%d" % i])
+            assert np.array_equal(np.array([b[:6] for b in lay], dtype=np.int64), z["layout_%d" % i])
+            x = np.random.default_rng(1000 + i).normal(size=nnz)
+            x /= np.linalg.norm(x)
+            y, d = np.zeros(nnz), np.zeros(nnz)
+            lib.dmrg_heff_apply(ctx, i, x, y)
+            lib.dmrg_heff_diag(ctx, i, d)
+            y0, d0 = z["y_%d" % i], z["diag_%d" % i]
+            assert np.linalg.norm(y - y0) <= 1e-11 * np.linalg.norm(y0)
+            assert np.abs(d - d0).max() <= 1e-11 * max(1.0, np.abs(d0).max())
+            st = lib.dmrg_heff_stats(ctx, i)
+            # flop accounting against the oracle's independent count: the oracle's literal term list
+            # (every enlarged operator a 4 x 4 grid, left factor first) never does fewer flops than the cheaper-order
+            # count over the library's list, and the two lists describe the same operator, so they stay within a small factor
+            f_or = float(z["gemm_flops_%d" % i])
+            assert 0 < st["f_exec"] <= st["f_alg"]
+            assert 0.2 * f_or <= st["f_alg"] <= 1.05 * f_or
+    finally:
+        lib.dmrg_destroy(ctx)
+
+
+@pytest.mark.parametrize("name", _files("sweep_cfg*_D*.json"))
+def test_sweep_vs_golden(lib, name):
+    gold = json.load(open(os.path.join(GOLD, name)))
+    cfg = make_config(gold["config"])
+    k, n, D = cfg["k"], cfg["n_elec"], gold["D"]
+    mps = random_mps(k, n, 0, gold["Dinit"], seed=gold["mps_seed"], gauge="R")
+    ctx = lib.dmrg_create(k, n, 0, cfg["h"], cfg["eri"], davidson_tol=gold["davidson_tol"])
+    try:
+        lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, 0)
+        for s, gs in enumerate(gold["sweeps"]):
+            r = lib.dmrg_sweep(ctx, D, k)
+            assert abs(r["energy_last"] - gs["energy_last"]) <= 1e-8
+            assert abs(r["energy_min"] - gs["energy_min"]) <= 1e-8
+            assert len(r["bonds"]) == len(gs["bonds"])
+            for rg, ro in zip(r["bonds"], gs["bonds"]):
+                assert rg["bond"] == ro["bond"] and rg["forward"] == (1 if ro["dir"] == "fwd" else 0)
+                assert abs(rg["energy"] - ro["energy"]) <= 1e-8, (s, ro["bond"], ro["dir"])
+                assert rg["kept"] == ro["kept"] and rg["nsectors"] == ro["nsectors"] and rg["nnz"] == ro["nnz"]
+                assert abs(rg["trunc_err"] - ro["trunc_err"]) <= 1e-9
+    finally:
+        lib.dmrg_destroy(ctx)
+
+
+@pytest.mark.parametrize("name", _files("rdm_cfg*_D*.npz"))
+def test_rdm_vs_golden(lib, name):
+    z = np.load(os.path.join(GOLD, name), allow_pickle=False)
+    cid, D = int(z["config"]), int(z["D"])
+    cfg = make_config(cid)
+    k, n = cfg["k"], cfg["n_elec"]
+    mps = random_mps(k, n, 0, D, seed=int(z["mps_seed"]), gauge="R")
+    ctx = lib.dmrg_create(k, n, 0, cfg["h"], cfg["eri"])
+    try:
+        lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, 0)
+        g, G = lib.dmrg_rdm12(ctx, k, True)
+    finally:
+        lib.dmrg_destroy(ctx)
+    assert np.abs(g - z["gamma"]).max() <= 1e-10
+    assert np.abs(G - z["Gamma"]).max() <= 1e-10
+    assert abs(np.trace(g) - n) <= 1e-10

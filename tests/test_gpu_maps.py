@@ -1,8 +1,6 @@
 """Device-built block maps against the host reference builder of the same library: the layout,
 the flop / byte accounting and the diagonal must agree exactly, H_eff x to rounding (the two builders order the
 K-concatenated segments differently), and both must match the oracle (tests/test_gpu_heff.py covers the default path)."""
-import os
-
 import numpy as np
 import pytest
 
@@ -12,15 +10,7 @@ pytestmark = pytest.mark.gpu
 
 
 def _run(lib, host_maps, k, n, s2, D, i, h, eri, mps, x):
-    old = os.environ.get("DMRG_B200_HOST_MAPS")
-    os.environ["DMRG_B200_HOST_MAPS"] = "1" if host_maps else "0"
-    try:
-        ctx = lib.dmrg_create(k, n, s2, h, eri, workspace_bytes=1 << 22)      # small workspace: several chunks
-    finally:
-        if old is None:
-            del os.environ["DMRG_B200_HOST_MAPS"]
-        else:
-            os.environ["DMRG_B200_HOST_MAPS"] = old
+    ctx = lib.dmrg_create(k, n, s2, h, eri, workspace_bytes=1 << 22, host_maps=1 if host_maps else 0)   # small workspace: several chunks
     try:
         lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, s2)
         lib.dmrg_prepare_bond(ctx, i)

@@ -100,3 +100,54 @@ def test_config1_untruncated_reaches_golden_fci(lib):
     assert np.abs(occ - np.array(gold["natural_occupations"])).max() <= 1e-6
     e_rdm = np.einsum("pq,pq->", cfg["h"], g) + 0.5 * np.einsum("pqrs,pqrs->", cfg["eri"], G)
     assert abs(e_rdm - gold["e_el_fci"][0]) <= 1e-8
+
+
+@pytest.mark.parametrize("opts", [dict(env_stride=3), dict(env_stride=2, host_spill=1), dict(env_stride=1, host_spill=1),
+                                  dict(env_stride=4, host_spill=1)])
+def test_sweep_env_checkpoints_and_host_spill_are_bit_identical(lib, opts):
+    """Environment-stack memory path: keeping only every env_stride-th block (the others recomputed when
+    a pass reaches them) and spilling the checkpoints to pinned host memory must not change a single bit of a sweep,
+    and must lower the peak device footprint."""
+    k, n, s2, D = 10, 10, 0, 48
+    h, eri = random_dense(k, 311)
+    mps = random_mps(k, n, s2, D, seed=41, gauge="R")
+    runs = []
+    for o in (dict(env_stride=1), opts):
+        ctx = lib.dmrg_create(k, n, s2, h, eri, davidson_tol=1e-10, **o)
+        try:
+            lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, s2)
+            base = lib.dmrg_device_bytes(ctx)
+            recs = [lib.dmrg_sweep(ctx, D, k) for _ in range(2)]
+            runs.append((recs, lib.dmrg_sweep_stats(ctx), base))
+        finally:
+            lib.dmrg_destroy(ctx)
+    (ra, sa, ba), (rb, sb, bb) = runs
+    for x, y in zip(ra, rb):
+        assert x["energy_last"] == y["energy_last"] and x["energy_min"] == y["energy_min"]
+        for bx, by in zip(x["bonds"], y["bonds"]):
+            assert bx["energy"] == by["energy"] and bx["kept"] == by["kept"] and bx["trunc_err"] == by["trunc_err"]
+    assert sb["env_stride"] == opts["env_stride"] and sb["host_spill"] == opts.get("host_spill", 0)
+    assert sb["peak_device_bytes"] - bb < sa["peak_device_bytes"] - ba
+    if opts.get("host_spill"):
+        assert sb["bytes_spilled"] > 0 and sb["bytes_restored"] > 0 and sb["host_pool_bytes"] > 0
+    else:
+        assert sb["seconds_regrow"] > 0
+
+
+def test_sweep_releases_consumed_environments(lib):
+    """With every block kept (env_stride = 1) a pass still frees what it has consumed: at the turn-around only one
+    operator stack is resident, so the peak is far below two stacks (round-1 behaviour)."""
+    k, n, s2, D = 12, 12, 0, 64
+    h, eri = random_dense(k, 77)
+    mps = random_mps(k, n, s2, D, seed=9, gauge="R")
+    ctx = lib.dmrg_create(k, n, s2, h, eri, env_stride=1)
+    try:
+        lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, s2)
+        base = lib.dmrg_device_bytes(ctx)
+        lib.dmrg_sweep(ctx, D, k)
+        after_first = lib.dmrg_device_bytes(ctx) - base           # = the right stack R_2 .. R_k
+        lib.dmrg_sweep(ctx, D, k)
+        st = lib.dmrg_sweep_stats(ctx)
+        assert st["peak_device_bytes"] - base < 1.6 * after_first
+    finally:
+        lib.dmrg_destroy(ctx)
