@@ -167,11 +167,18 @@ int dmrg_sweep_stats(dmrg_ctx* ctx, dmrg_sweep_stats_t* out);
  * the results are in place. */
 int dmrg_rdm12(dmrg_ctx* ctx, double* gamma, double* Gamma, int where, void* cuda_stream);
 
-/* Timing / accounting of the last dmrg_rdm12 call: seconds of the whole pass, bytes of operator storage streamed by
- * the accumulation kernels (E = Stack M^T: every stored operator once per centre, plus the M vectors), all flops, and
- * the device seconds (CUDA events) of those accumulation kernels alone, so that bytes_streamed / stream_seconds is
- * their achieved HBM rate.  Any output pointer may be null. */
-int dmrg_rdm_stats(dmrg_ctx* ctx, double* seconds, double* bytes_streamed, double* flops, double* stream_seconds);
+/* Timing / accounting of the last dmrg_rdm12 call.  bytes_streamed: operator storage (plus the M
+ * vectors) read by ALL accumulation launches E = Stack M^T - every stored operator of the two-index side once per
+ * centre; of these, stream_bytes went through the HBM-bound streaming kernel (operator classes with <= 8 right-hand
+ * sides) in stream_seconds of device time (CUDA events), the rest through split-K launches of the FP64 tensor-pipe GEMM in
+ * gemm_seconds.  seconds_host: string enumeration and gamma / Gamma scatter on the host; seconds_renormalise: centre
+ * moves and blocking steps of the pass (host plan assembly + kernels). */
+typedef struct dmrg_rdm_stats_t {
+    double seconds, seconds_host, seconds_renormalise;
+    double bytes_streamed, flops;
+    double stream_bytes, stream_seconds, gemm_seconds;
+} dmrg_rdm_stats_t;
+int dmrg_rdm_stats(dmrg_ctx* ctx, dmrg_rdm_stats_t* out);
 
 /* Number of kernels this library launched on the context since creation (bench.py's gpu_launches). */
 int64_t dmrg_launch_count(const dmrg_ctx* ctx);

@@ -227,10 +227,15 @@ def dmrg_rdm12(ctx, k, want_2rdm=True, out=None):
     return g, G
 
 
+class dmrg_rdm_stats_t(C.Structure):
+    _fields_ = [(n, C.c_double) for n in ("seconds", "seconds_host", "seconds_renormalise", "bytes_streamed", "flops",
+                                          "stream_bytes", "stream_seconds", "gemm_seconds")]
+
+
 def dmrg_rdm_stats(ctx):
-    s, b, f, t = C.c_double(), C.c_double(), C.c_double(), C.c_double()
-    _check(ctx, lib.dmrg_rdm_stats(ctx, C.byref(s), C.byref(b), C.byref(f), C.byref(t)))
-    return dict(seconds=s.value, bytes_streamed=b.value, flops=f.value, stream_seconds=t.value)
+    st = dmrg_rdm_stats_t()
+    _check(ctx, lib.dmrg_rdm_stats(ctx, C.byref(st)))
+    return dict((f, getattr(st, f)) for f, _ in dmrg_rdm_stats_t._fields_)
 
 
 def dmrg_launch_count(ctx):

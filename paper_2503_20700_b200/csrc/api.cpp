@@ -419,12 +419,13 @@ int dmrg_rdm12(dmrg_ctx* ctx, double* gamma, double* Gamma, int where, void* cud
     API_END
 }
 
-int dmrg_rdm_stats(dmrg_ctx* ctx, double* seconds, double* bytes_streamed, double* flops, double* stream_seconds) {
+int dmrg_rdm_stats(dmrg_ctx* ctx, dmrg_rdm_stats_t* out) {
     API_BEGIN(ctx)
-    if (seconds) *seconds = eng.rdm_seconds;
-    if (bytes_streamed) *bytes_streamed = eng.rdm_bytes;
-    if (flops) *flops = eng.rdm_flops;
-    if (stream_seconds) *stream_seconds = eng.rdm_stream_ms * 1e-3;
+    if (!out) return fail(eng, DMRG_EINVAL, "rdm_stats: null output");
+    out->seconds = eng.rdm_seconds; out->seconds_host = eng.rdm_host_seconds; out->seconds_renormalise = eng.rdm_grow_seconds;
+    out->bytes_streamed = eng.rdm_bytes; out->flops = eng.rdm_flops;
+    out->stream_bytes = eng.rdm_stream_bytes; out->stream_seconds = eng.rdm_stream_ms * 1e-3;
+    out->gemm_seconds = eng.rdm_gemm_ms * 1e-3;
     return DMRG_OK;
     API_END
 }

@@ -175,9 +175,10 @@ void make_temps(const Ham& ham, Block& X, const Dot& dot, const std::vector<int>
 std::unique_ptr<Block> empty_block(char side, int k, const MPS& mps);
 // one blocking step with the tensor of the neighbouring site (fused form-and-rotate)
 std::unique_ptr<Block> grow(Block& X, const Ham& ham, const MPS& mps, char new_mode, Engine& eng);
-// blocking step that keeps only a+_P (and optionally A, B): what the RDM pass needs
+// blocking step that keeps only a+_P of every inside orbital and A_PQ, B_PS of the pairs whose two SITES both lie in
+// [pair_lo, pair_hi) (empty range: one-index operators only): what the RDM pass needs
 std::unique_ptr<Block> grow_normal(Block& X, const Ham& ham, const Basis& new_basis, const SiteTensor& tensor,
-                                   bool two_index, Engine& eng);
+                                   int pair_lo, int pair_hi, Engine& eng);
 BlockInfo block_info(const Block& b);
 
 // ---- H_eff ---------------------------------------------------------------------------------------------------------
@@ -250,7 +251,8 @@ struct Engine {
     double flops_total = 0;                       // unpadded flops of every grouped-GEMM launch since creation
     std::string last_error;
     SvdWork* svd = nullptr;
-    double rdm_seconds = 0, rdm_bytes = 0, rdm_flops = 0;
+    double rdm_seconds = 0, rdm_bytes = 0, rdm_flops = 0, rdm_host_seconds = 0, rdm_grow_seconds = 0, rdm_gemm_ms = 0;
+    double rdm_stream_bytes = 0;                  // bytes of the launches of the HBM-bound streaming kernel alone
     double t_plan = 0, t_davidson = 0, t_split = 0, t_grow = 0, t_matvec = 0;   // phase seconds of the last sweep
     double rdm_stream_ms = 0;                     // device time of the operator-streaming kernels (E = Stack M^T) alone
     bool keep_env_stack = true;

@@ -293,19 +293,22 @@ std::unique_ptr<Block> grow(Block& X, const Ham& ham, const MPS& mps, char new_m
 }
 
 std::unique_ptr<Block> grow_normal(Block& X, const Ham& ham, const Basis& new_basis, const SiteTensor& tensor,
-                                   bool two_index, Engine& eng) {
+                                   int pair_lo, int pair_hi, Engine& eng) {
     const bool left = X.side == 'L';
     const int p = left ? X.b : X.b - 1, nbond = left ? X.b + 1 : X.b - 1;
     Dot dot(&ham, std::vector<int>{p});
     std::unique_ptr<Block> nbp(new Block(X.side, nbond, X.k, new_basis, 'N'));
     Gen gen(ham, block_info(X), dot);
     const std::vector<int> inside = nbp->inside();
+    auto paired = [&](int P) { const int s = P >> 1; return s >= pair_lo && s < pair_hi; };
     std::vector<NewOp> list;
     for (size_t a = 0; a < inside.size(); ++a) {
         list.push_back({L1(K_C, inside[a]), gen.cre(inside[a])});
-        if (!two_index) continue;
-        for (size_t b = a + 1; b < inside.size(); ++b) list.push_back({L2(K_A, inside[a], inside[b]), gen.A(inside[a], inside[b])});
-        for (int S : inside) list.push_back({L2(K_B, inside[a], S), gen.B(inside[a], S)});
+        if (!paired(inside[a])) continue;
+        for (size_t b = a + 1; b < inside.size(); ++b)
+            if (paired(inside[b])) list.push_back({L2(K_A, inside[a], inside[b]), gen.A(inside[a], inside[b])});
+        for (int S : inside)
+            if (paired(S)) list.push_back({L2(K_B, inside[a], S), gen.B(inside[a], S)});
     }
     rotate_batch(X, dot, tensor, *nbp, list, false, eng);
     return nbp;
