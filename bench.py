@@ -44,11 +44,19 @@ def parse_args():
     ap.add_argument("--config", type=int, default=4, help="BASELINE config 1..5 (default 4: the metric's workload)")
     ap.add_argument("--D", type=int, default=0, help="bond dimension override (0 = the config's)")
     ap.add_argument("--bond", type=int, default=-1, help="two-site bond (default mid-chain k/2-1)")
-    ap.add_argument("--extras", type=int, default=2, help="1: also time sweeps + RDM on config 1; 2: on configs 1-3; 3: + one sweep of config 4 at D=1024")
+    ap.add_argument("--extras", type=int, default=2, help="1: also time sweeps + RDM on config 1; 2: on configs 1-3")
+    ap.add_argument("--big", type=int, default=0, help="4 or 5: only time sweeps + the RDM pass of that config at --sweep-D (memory path)")
+    ap.add_argument("--sweeps", type=int, default=1)
+    ap.add_argument("--rdm", type=int, default=1)
+    ap.add_argument("--max-iter", type=int, default=12, help="Davidson iterations per bond of --big sweeps")
+    ap.add_argument("--host-spill", type=int, default=1)
+    ap.add_argument("--env-stride", type=int, default=0)
+    ap.add_argument("--hbm-budget-gb", type=float, default=0.0)
+    ap.add_argument("--host-budget-gb", type=float, default=0.0)
     ap.add_argument("--cpu-baseline", type=int, default=1)
     ap.add_argument("--sample-config", type=int, default=2, help="config of the oracle's bounded sample")
     ap.add_argument("--sample-D", type=int, default=96)
-    ap.add_argument("--sweep-D", type=int, default=1024, help="bond dimension of the config-4 sweep of --extras 3")
+    ap.add_argument("--sweep-D", type=int, default=2048, help="bond dimension of the --big sweeps")
     ap.add_argument("--workspace-gb", type=float, default=0.0, help="intermediate workspace of H_eff psi (0 = library default)")
     ap.add_argument("--probe", type=int, default=1, help="1: run the FP64 ceiling probes (DMMA, DFMA, LDS-fed DMMA, cuBLAS DGEMM)")
     return ap.parse_args()
@@ -216,58 +224,97 @@ def run_reference(args):
     print(json.dumps(line))
 
 
-def time_small_extras(P, torch, peaks, level, sweep_D=1024):
-    """Seconds per sweep and 1-/2-RDM time on BASELINE configs 1 (D = 64), 2 (D = 512) and 3 (D = 1024): the remaining
-    rows of the hot path (a1, a3, a4, a5, a6) exercised end to end in the same run.  level 1: config 1 only; 2: configs
-    1-3 with one sweep each (from a seeded random MPS, so bond dimensions are saturated from the start)."""
+def time_sweep_rdm(P, torch, peaks, cid, D, nsweep, rdm=True, **opts):
+    """Seconds per sweep (with the phase breakdown and the environment-stack accounting of dmrg_sweep_stats) and the
+    1-/2-RDM pass (dmrg_rdm_stats) of BASELINE config `cid` at bond dimension D, from a seeded random MPS of that D (bond
+    dimensions saturated from the start).  opts: dmrg_options fields (davidson_max_iter, host_spill, env_stride, ...)."""
     from synth import make_config, random_mps, mps_to_blob_arrays
-    out = {}
-    plan = [(1, 3, 0), (2, 1, 0), (3, 1, 0), (4, 1, sweep_D)]  # (config, sweeps, D override); config 4 at reduced D: the
-    for cid, nsweep, Dov in plan[: {1: 1, 2: 3}.get(level, 4)]:  # environment stack of D = 4096 does not fit one GPU yet
-        cfg = make_config(cid)
-        k, n, D = cfg["k"], cfg["n_elec"], Dov or cfg["D"]
-        mps = random_mps(k, n, 0, D, seed=cfg["seed"] + 1000, gauge="R")
-        ctx = P.dmrg_create(k, n, 0, cfg["h"], cfg["eri"])
-        rec = {"workload": "%s D=%d" % (cfg["name"], D)}
+    cfg = make_config(cid)
+    k, n = cfg["k"], cfg["n_elec"]
+    mps = random_mps(k, n, 0, D, seed=cfg["seed"] + 1000, gauge="R")
+    ctx = P.dmrg_create(k, n, 0, cfg["h"], cfg["eri"], **opts)
+    rec = {"workload": "%s D=%d" % (cfg["name"], D), "options": opts}
+    try:
+        P.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, 0)
+        del mps
+        secs, e, r, phases = [], None, None, []
         try:
-            P.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, 0)
-            secs, e, r = [], None, None
-            try:
-                for _ in range(nsweep):
-                    r = P.dmrg_sweep(ctx, D, k)
-                    secs.append(r["seconds"])
-                    e = r["energy_last"]
-            except P.binding.DmrgError as ex:                 # e.g. the environment stack does not fit the device
-                rec["sweep"] = {"error": str(ex), "s_per_sweep": secs}
-                out["config%d" % cid] = rec
-                continue
-            mv = int(sum(b["n_matvec"] for b in r["bonds"]))
-            fl = float(sum(b["n_matvec"] * b["f_alg"] for b in r["bonds"]))
-            tmv = float(sum(b["seconds_matvec"] for b in r["bonds"]))
-            rec["sweep"] = {"s_per_sweep": secs, "energy_last_eh": e + cfg["e_core"], "matvecs_last_sweep": mv,
-                            "matvec_seconds_last_sweep": tmv, "matvec_f_alg_last_sweep": fl,
-                            "matvec_tflops_last_sweep": fl / tmv / 1e12 if tmv > 0 else None,
-                            "max_kept": int(max(b["kept"] for b in r["bonds"]))}
-            if cid > 3:
-                rec["rdm12"] = {"skipped": "the round-1 RDM pass keeps all two-index operators of one side (DESIGN.md 5.4)"}
-                out["config%d" % cid] = rec
-                continue
-            try:
-                t0 = time.perf_counter()
-                g, G = P.dmrg_rdm12(ctx, k, True)
-                torch.cuda.synchronize()
-                st = P.dmrg_rdm_stats(ctx)
-                gbs = st["bytes_streamed"] / st["stream_seconds"] / 1e9 if st["stream_seconds"] > 0 else None
-                rec["rdm12"] = {"seconds": time.perf_counter() - t0, "device_seconds": st["seconds"],
-                                "trace_gamma": float(np.trace(g)), "gbytes_streamed": st["bytes_streamed"] / 1e9,
-                                "stream_seconds": st["stream_seconds"], "stream_gbs": gbs,
-                                "stream_frac_of_hbm": gbs / peaks["hbm"] if gbs else None, "flops": st["flops"]}
-            except P.binding.DmrgError as ex:
-                rec["rdm12"] = {"error": str(ex)}
-        finally:
-            P.dmrg_destroy(ctx)
-        out["config%d" % cid] = rec
+            for _ in range(nsweep):
+                r = P.dmrg_sweep(ctx, D, k)
+                secs.append(r["seconds"])
+                e = r["energy_last"]
+                phases.append(P.dmrg_sweep_stats(ctx))
+        except P.binding.DmrgError as ex:                 # e.g. the environment stack does not fit the device
+            rec["sweep"] = {"error": str(ex), "s_per_sweep": secs}
+            return rec
+        mv = int(sum(b["n_matvec"] for b in r["bonds"]))
+        fl = float(sum(b["n_matvec"] * b["f_alg"] for b in r["bonds"]))
+        tmv = float(sum(b["seconds_matvec"] for b in r["bonds"]))
+        rec["sweep"] = {"s_per_sweep": secs, "energy_last_eh": e + cfg["e_core"], "matvecs_last_sweep": mv,
+                        "matvec_seconds_last_sweep": tmv, "matvec_f_alg_last_sweep": fl,
+                        "matvec_tflops_last_sweep": fl / tmv / 1e12 if tmv > 0 else None,
+                        "max_kept": int(max(b["kept"] for b in r["bonds"])),
+                        "unconverged_bonds": int(sum(1 - b["converged"] for b in r["bonds"])),
+                        "phases_last_sweep": phases[-1]}
+        if not rdm:
+            return rec
+        try:
+            t0 = time.perf_counter()
+            g, G = P.dmrg_rdm12(ctx, k, True)
+            torch.cuda.synchronize()
+            wall = time.perf_counter() - t0
+            st = P.dmrg_rdm_stats(ctx)
+            gbs = st["stream_bytes"] / st["stream_seconds"] / 1e9 if st["stream_seconds"] > 0 else None
+            kern = st["stream_seconds"] + st["gemm_seconds"]
+            e_rdm = float(np.einsum("pq,pq->", cfg["h"], g) + 0.5 * np.einsum("pqrs,pqrs->", cfg["eri"], G))
+            rec["rdm12"] = {"seconds": wall, "trace_gamma": float(np.trace(g)),
+                            "partial_trace_err": float(np.abs(np.einsum("pqrr->pq", G) - (n - 1) * g).max()),
+                            "e_rdm_eh": e_rdm + cfg["e_core"],
+                            "seconds_host_scatter": st["seconds_host"], "seconds_renormalise": st["seconds_renormalise"],
+                            "accumulation_gbytes": st["bytes_streamed"] / 1e9, "accumulation_kernel_seconds": kern,
+                            "accumulation_gbs": st["bytes_streamed"] / kern / 1e9 if kern > 0 else None,
+                            "stream_kernel_gbytes": st["stream_bytes"] / 1e9, "stream_kernel_seconds": st["stream_seconds"],
+                            "stream_kernel_gbs": gbs, "stream_kernel_frac_of_hbm": gbs / peaks["hbm"] if gbs else None,
+                            "gemm_kernel_seconds": st["gemm_seconds"], "flops": st["flops"]}
+        except P.binding.DmrgError as ex:
+            rec["rdm12"] = {"error": str(ex)}
+    finally:
+        P.dmrg_destroy(ctx)
+    return rec
+
+
+def time_small_extras(P, torch, peaks, level):
+    """The remaining rows of the hot path (a1, a3, a4, a5, a6) end to end in the same run: seconds per sweep and 1-/2-RDM
+    time on BASELINE configs 1 (D = 64, 3 sweeps), 2 (D = 512) and 3 (D = 1024).  level 1: config 1 only."""
+    out = {}
+    for cid, nsweep in [(1, 3), (2, 1), (3, 1)][: 1 if level == 1 else 3]:
+        out["config%d" % cid] = time_sweep_rdm(P, torch, peaks, cid, {1: 64, 2: 512, 3: 1024}[cid], nsweep)
     return out
+
+
+def run_big(args):
+    """`--big C`: one line with seconds per sweep and the RDM pass of BASELINE config C (4 or 5) at --sweep-D through the
+    environment-stack memory path (checkpoints, recomputation, pinned-host spill); minutes of GPU time, not part of the
+    default run.  Davidson is capped at --max-iter iterations per bond: from a random MPS an uncapped first sweep needs
+    ~50 matvecs per bond, a converged calculation ~10 (the matvec count is reported)."""
+    import torch
+    import __graft_entry__ as entry
+    entry.build()
+    import paper_2503_20700_b200 as P
+    torch.cuda.set_device(0)
+    peaks = measured_peaks()
+    opts = dict(davidson_max_iter=args.max_iter, host_spill=args.host_spill, env_stride=args.env_stride)
+    if args.hbm_budget_gb > 0:
+        opts["hbm_budget_bytes"] = int(args.hbm_budget_gb * (1 << 30))
+    if args.host_budget_gb > 0:
+        opts["host_budget_bytes"] = int(args.host_budget_gb * (1 << 30))
+    if args.workspace_gb > 0:
+        opts["workspace_bytes"] = int(args.workspace_gb * (1 << 30))
+    sampler = ClockSampler(0)
+    sampler.start()
+    rec = time_sweep_rdm(P, torch, peaks, args.big, args.sweep_D, args.sweeps, rdm=bool(args.rdm), **opts)
+    rec["clocks"] = sampler.stop()
+    print(json.dumps({"big": rec}))
 
 
 def run_ours(args):
@@ -411,7 +458,7 @@ def run_ours(args):
         del S
         torch.cuda.profiler.stop()
     if args.extras:
-        line["extras"] = time_small_extras(P, torch, peaks, args.extras, args.sweep_D)
+        line["extras"] = time_small_extras(P, torch, peaks, args.extras)
     if args.cpu_baseline and world == 1:
         v, info = oracle_sample(args, 3, 1)
         line["cpu_baseline"] = dict(info, value=v, unit=UNIT)
@@ -422,6 +469,8 @@ def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.big:
+        run_big(args)
     else:
         run_ours(args)
     if int(os.environ.get("WORLD_SIZE", 1)) > 1:

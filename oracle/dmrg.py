@@ -713,10 +713,42 @@ def davidson(apply, diag, x0, tol=1e-7, max_iter=100, max_subspace=20):
 # ----------------------------------------------------------------------------------------------------------------
 # decomposition and truncation (reading S14) and the two-site sweep (readings S12, S16-S18)
 # ----------------------------------------------------------------------------------------------------------------
-def split_theta(theta_blocks, bonds_l, bonds_r, D, direction, sv_floor=1e-10, cluster_rel_gap=1e-6):
-    """SVD of the two-site tensor per enlarged-left sector, global top-D selection that never cuts through a
-    near-degenerate cluster.  Returns (mid_basis, A blocks {(l,a): [d_l,d_m]}, B blocks {(m,b): [d_m,d_r]},
-    trunc_err, kept) with singular values absorbed to the right ('fwd') or to the left ('bwd')."""
+def select_kept(sv_sorted, D, sv_floor=1e-10, cluster_rel_gap=1e-6, dbss_eps=0.0, dbss_dmin=0):
+    """Number of kept states from the pooled singular values of the normalised two-site state, sorted descending.
+    Fixed D (reading S14): m = min(D, #sigma > floor); while the cut falls inside a near-degenerate cluster
+    (sigma_{m+1} >= (1 - gap) sigma_m) decrease m; if that empties the bond keep the original m.
+    DBSS (fixed truncation error eps_TR with a minimal bond dimension D_min; reading S32):
+    m_eps = the fewest states whose discarded weight 1 - sum_{t < m} sigma_t^2 is <= eps_TR, then
+    m = min(max(m_eps, D_min), D_max = D, #sigma > floor); a cut inside a cluster is moved UP to the end of the
+    cluster when that stays within min(D_max, count) (the error target stays met), otherwise down as in S14."""
+    count = sum(1 for sv in sv_sorted if sv > sv_floor)
+    cap = min(D, count)
+    inside = lambda m: 0 < m < count and sv_sorted[m] >= (1.0 - cluster_rel_gap) * sv_sorted[m - 1]
+    if dbss_eps > 0.0:
+        kept_w, m = 0.0, 0
+        while m < count and 1.0 - kept_w > dbss_eps:
+            kept_w += sv_sorted[m] ** 2
+            m += 1
+        m = min(max(m, dbss_dmin), cap)
+        up = m
+        while inside(up):
+            up += 1
+        if up <= cap:
+            return up
+    else:
+        m = cap
+    m0 = m
+    while inside(m):
+        m -= 1
+    return m0 if m == 0 else m
+
+
+def split_theta(theta_blocks, bonds_l, bonds_r, D, direction, sv_floor=1e-10, cluster_rel_gap=1e-6, dbss_eps=0.0,
+                dbss_dmin=0):
+    """SVD of the two-site tensor per enlarged-left sector, global selection of the kept states by select_kept (fixed
+    D or DBSS; never cuts through a near-degenerate cluster).  Returns (mid_basis, A blocks {(l,a): [d_l,d_m]},
+    B blocks {(m,b): [d_m,d_r]}, trunc_err, kept) with singular values absorbed to the right ('fwd') or to the left
+    ('bwd')."""
     rindex = {(n, s): j for j, (n, s, d) in enumerate(bonds_r)}
     sectors = {}
     for (li, a, b), blk in theta_blocks.items():
@@ -754,13 +786,7 @@ def split_theta(theta_blocks, bonds_l, bonds_r, D, direction, sv_floor=1e-10, cl
             pool.append((sv, q, j))
     order = sorted(range(len(pool)), key=lambda t: -pool[t][0])       # stable: ties by (sector, index)
     sv_sorted = [pool[t][0] for t in order]
-    count = sum(1 for sv in sv_sorted if sv > sv_floor)
-    m = min(D, count)
-    m0 = m
-    while 0 < m < count and sv_sorted[m] >= (1.0 - cluster_rel_gap) * sv_sorted[m - 1]:
-        m -= 1
-    if m == 0:
-        m = m0
+    m = select_kept(sv_sorted, D, sv_floor, cluster_rel_gap, dbss_eps, dbss_dmin)
     keep = {}
     for t in order[:m]:
         _, q, j = pool[t]
@@ -803,7 +829,8 @@ class SweepEngine:
     """Two-site fixed-D DMRG on an imported right-canonical MPS (C3 step 4).  One call of sweep() = forward pass
     over bonds 0..k-2 then backward pass k-2..0 (reading S12)."""
 
-    def __init__(self, h, eri, mps, davidson_tol=1e-7, davidson_max_iter=100, davidson_max_subspace=20):
+    def __init__(self, h, eri, mps, davidson_tol=1e-7, davidson_max_iter=100, davidson_max_subspace=20, dbss_eps=0.0,
+                 dbss_dmin=0):
         self.ham = Ham(h, eri)
         self.k = self.ham.k
         self.mps = dict(mps)
@@ -811,6 +838,7 @@ class SweepEngine:
         self.mps["tensors"] = [dict(t) for t in mps["tensors"]]
         self.mps["gauge"] = list(mps["gauge"])
         self.opts = dict(tol=davidson_tol, max_iter=davidson_max_iter, max_subspace=davidson_max_subspace)
+        self.dbss = dict(dbss_eps=dbss_eps, dbss_dmin=dbss_dmin)
         self.L = {0: empty_block("L", self.k, self.mps)}
         self.R = build_right(self.mps, self.ham, 2)
         self.log = []
@@ -821,7 +849,7 @@ class SweepEngine:
         guess = blocks_to_flat(H.layout, H.nnz, two_site_tensor(mps, i))
         theta, u, nmv, rn, ok = davidson(H.apply, H.diagonal(), guess, **self.opts)
         ub = flat_to_blocks(H.layout, u)
-        mid, Ab, Bb, trunc, kept = split_theta(ub, mps["bonds"][i], mps["bonds"][i + 2], D, direction)
+        mid, Ab, Bb, trunc, kept = split_theta(ub, mps["bonds"][i], mps["bonds"][i + 2], D, direction, **self.dbss)
         mps["bonds"][i + 1] = mid
         mps["tensors"][i], mps["tensors"][i + 1] = Ab, Bb
         if direction == "fwd":

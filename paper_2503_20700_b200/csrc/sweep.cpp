@@ -249,10 +249,27 @@ void split_theta(MPS& mps, int i, const HeffPlan& p, const double* theta, int D,
     std::stable_sort(idx.begin(), idx.end(), [&](int x, int y) { return pool[x].sv > pool[y].sv; });
     int count = 0;
     for (int t : idx) if (pool[t].sv > eng.opt.sv_floor) ++count;
-    int m = std::min(D, count);
-    const int m0 = m;
-    while (m > 0 && m < count && pool[idx[m]].sv >= (1.0 - eng.opt.cluster_rel_gap) * pool[idx[m - 1]].sv) --m;
-    if (m == 0) m = m0;
+    // kept states: fixed D (reading S14) or dynamic block state selection (reading S32: the
+    // fewest states with discarded weight <= dbss_eps, clamped to [dbss_dmin, D]); a cut never splits a near-degenerate
+    // cluster - under DBSS it moves up to the end of the cluster when the cap allows, otherwise (and for fixed D) down
+    const int cap = std::min(D, count);
+    auto inside = [&](int mm) { return mm > 0 && mm < count && pool[idx[mm]].sv >= (1.0 - eng.opt.cluster_rel_gap) * pool[idx[mm - 1]].sv; };
+    int m = cap;
+    bool chosen = false;
+    if (eng.opt.dbss_eps > 0.0) {
+        double kw = 0.0;
+        m = 0;
+        while (m < count && 1.0 - kw > eng.opt.dbss_eps) { kw += pool[idx[m]].sv * pool[idx[m]].sv; ++m; }
+        m = std::min(std::max(m, eng.opt.dbss_dmin), cap);
+        int up = m;
+        while (inside(up)) ++up;
+        if (up <= cap) { m = up; chosen = true; }
+    }
+    if (!chosen) {
+        const int m0 = m;
+        while (inside(m)) --m;
+        if (m == 0) m = m0;
+    }
     if (m == 0) throw Error(-2, "split: the two-site state has no singular value above the floor");
     double kept_w = 0.0;
     for (int t = 0; t < m; ++t) { kept_w += pool[idx[t]].sv * pool[idx[t]].sv; order[pool[idx[t]].sec]->keep++; }

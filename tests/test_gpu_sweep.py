@@ -151,3 +151,26 @@ def test_sweep_releases_consumed_environments(lib):
         assert st["peak_device_bytes"] - base < 1.6 * after_first
     finally:
         lib.dmrg_destroy(ctx)
+
+
+@pytest.mark.parametrize("k,n,s2,eps,dmin,dmax", [(6, 6, 0, 1e-6, 6, 40), (8, 8, 0, 1e-5, 10, 32), (8, 9, 1, 1e-4, 4, 64)])
+def test_dbss_sweep_matches_oracle(lib, k, n, s2, eps, dmin, dmax):
+    """Dynamic block state selection (reading S32): kept states per bond, truncation error and
+    energies of DBSS sweeps, device vs oracle."""
+    h, eri = random_dense(k, 400 + k)
+    mps = random_mps(k, n, s2, 16, seed=55 + k, gauge="R")
+    ctx = lib.dmrg_create(k, n, s2, h, eri, davidson_tol=1e-10, dbss_eps=eps, dbss_dmin=dmin)
+    eng = odmrg.SweepEngine(h, eri, mps, davidson_tol=1e-10, dbss_eps=eps, dbss_dmin=dmin)
+    try:
+        lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, s2)
+        kept = set()
+        for _ in range(3):
+            g, o = lib.dmrg_sweep(ctx, dmax, k), eng.sweep(dmax)
+            assert abs(g["energy_last"] - o["energy_last"]) <= TOL_E
+            for rg, ro in zip(g["bonds"], o["bonds"]):
+                assert rg["kept"] == ro["kept"] and rg["nsectors"] == ro["nsectors"]
+                assert abs(rg["energy"] - ro["energy"]) <= TOL_E and abs(rg["trunc_err"] - ro["trunc_err"]) <= 1e-9
+                kept.add(rg["kept"])
+        assert len(kept) > 2                                      # the bond dimension really varies along the chain
+    finally:
+        lib.dmrg_destroy(ctx)

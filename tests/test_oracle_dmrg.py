@@ -4,7 +4,7 @@ import numpy as np
 import pytest
 
 from oracle import fci, dmrg
-from synth import random_dense, random_mps, make_config
+from synth import random_dense, random_mps, make_config, full_sector_dims
 
 
 @pytest.mark.parametrize("k,n,s2,D", [(4, 4, 0, 8), (5, 5, 1, 10), (6, 8, 0, 12), (6, 3, -1, 12)])
@@ -126,3 +126,53 @@ def test_config1_untruncated_sweep_vs_fci():
     for _ in range(3):
         r = eng.sweep(1024)
     assert abs(r["energy_last"] + cfg["e_core"] - (-0.8822829988)) < 1e-8
+
+
+def test_select_kept_fixed_D_and_dbss_on_synthetic_spectra():
+    """Pins of the truncation rule (readings S14, S32) on spectra where the answer is known by
+    hand: the kept count follows eps_TR, clamps at D_min / D_max, and never splits a near-degenerate cluster."""
+    sel = dmrg.select_kept
+    # geometric spectrum sigma_t^2 = w0 r^t, normalised: discarded weight after m states is r^m exactly
+    r = 0.5
+    sv = np.sqrt((1 - r) * r ** np.arange(80))
+    sv = list(sv / np.sqrt(np.sum(sv ** 2)))
+    for eps, want in [(0.3, 2), (0.2, 3), (1e-3, 10), (1e-6, 20)]:          # r^m <= eps  <=>  m >= log(eps) / log(r)
+        assert sel(sv, 1000, dbss_eps=eps) == want
+    assert sel(sv, 1000, dbss_eps=1e-3, dbss_dmin=16) == 16                  # clamps at D_min
+    assert sel(sv, 7, dbss_eps=1e-3) == 7                                    # clamps at D_max
+    assert sel(sv, 7, dbss_eps=1e-3, dbss_dmin=16) == 7                      # D_max wins over D_min
+    assert sel(sv, 12) == 12 and sel(sv, 1000) == 66                         # fixed D; sigma_t = 0.5^((t+1)/2) <= 1e-10 dropped
+    # clusters: doublets (sigma_{2j} = sigma_{2j+1}), as the Sz partners of a spin multiplet
+    w = np.repeat(0.5 ** np.arange(10), 2)
+    d = list(np.sqrt(w / w.sum()))
+    assert sel(d, 5) == 4 and sel(d, 6) == 6 and sel(d, 1) == 1              # fixed D: cut moves down, never to zero
+    disc = lambda m: 1.0 - sum(x * x for x in d[:m])
+    m = sel(d, 100, dbss_eps=disc(3) * 0.999)                                # target needs 4 states -> exactly a boundary
+    assert m == 4
+    m = sel(d, 100, dbss_eps=disc(3) * 1.001)                                # 3 states would do: inside a doublet -> up to 4
+    assert m == 4 and disc(m) <= disc(3)
+    assert sel(d, 3, dbss_eps=disc(3) * 1.001) == 2                          # cannot go up (D_max = 3): moves down
+    assert sel(d, 100, dbss_eps=0.9, dbss_dmin=5) == 6                       # D_min inside a doublet -> up
+
+
+def test_dbss_sweep_truncation_error_below_target():
+    """A DBSS sweep of the oracle keeps, at every bond, a truncation error <= eps_TR unless the bond sits at D_max, and
+    at least D_min states where the bond allows it; its energy lies between the D_min and the D_max fixed-D energies."""
+    k, n, s2 = 6, 6, 0
+    h, eri = random_dense(k, 5)
+    mps = random_mps(k, n, s2, 24, seed=3, gauge="R")
+    eps, dmin, dmax = 1e-6, 6, 40
+    eng = dmrg.SweepEngine(h, eri, mps, davidson_tol=1e-10, dbss_eps=eps, dbss_dmin=dmin)
+    for _ in range(3):
+        r = eng.sweep(dmax)
+    full = full_sector_dims(k, n, s2)
+    for b in r["bonds"]:
+        cap = min(dmax, sum(full[b["bond"] + 1].values()))
+        assert b["kept"] <= dmax
+        assert b["trunc_err"] <= eps * (1 + 1e-9) or b["kept"] >= cap - 3       # within a cluster of the cap
+        assert b["kept"] >= min(dmin, cap) - 3
+    lo = dmrg.SweepEngine(h, eri, mps, davidson_tol=1e-10)
+    hi = dmrg.SweepEngine(h, eri, mps, davidson_tol=1e-10)
+    for _ in range(3):
+        e_lo, e_hi = lo.sweep(dmin)["energy_last"], hi.sweep(dmax)["energy_last"]
+    assert e_hi - 1e-9 <= r["energy_last"] <= e_lo + 1e-9
