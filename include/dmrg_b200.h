@@ -191,11 +191,14 @@ int64_t dmrg_device_bytes(const dmrg_ctx* ctx);
 /* Kernel-level entry used by the unit parity tests: grouped, K-segmented FP64 GEMM on device buffers.
  * For task t: C_t[M x N] (+)= sum_{s in segs of t} alpha_s op(A_s) op(B_s); all pointers are DEVICE addresses
  * stored as int64; arrays below are HOST arrays (copied to the device by the call).  seg_flags bit0: A stored
- * [K x M]; bit1: B stored [N x K]; bit2: B = identity (C += alpha A, A stored [M x N]).  task_flags bit0: accumulate. */
+ * [K x M]; bit1: B stored [N x K]; bit2: B = identity (C += alpha A, A stored [M x N]).  task_flags bit0: accumulate.  generic_kernel
+ * != 0 forces the cp.async kernel (otherwise the bulk-copy kernel runs whenever the operands are aligned); *kernel_ms (HOST,
+ * nullable) receives the device time of the kernel launch alone (CUDA events on `cuda_stream`, descriptor upload excluded). */
 int dmrg_grouped_gemm(int ntasks, const int64_t* c_ptr, const int32_t* ldc, const int32_t* m, const int32_t* n,
                       const int32_t* seg_begin, const int32_t* seg_count, const int32_t* task_flags, int nsegs,
                       const int64_t* a_ptr, const int64_t* b_ptr, const int32_t* lda, const int32_t* ldb,
-                      const int32_t* kk, const int32_t* seg_flags, const double* alpha, void* cuda_stream);
+                      const int32_t* kk, const int32_t* seg_flags, const double* alpha, int generic_kernel,
+                      double* kernel_ms, void* cuda_stream);
 
 /* Kernel-level entry of the RDM accumulation kernel for few right-hand sides ("streams every stored
  * 2-index operator once", HBM-bound):  E[r*ldE + c] = sum_k S[r*lds + k] * M[c*ldm + k], r < nrows, c < nc (1..8), k < K.
@@ -204,19 +207,6 @@ int dmrg_grouped_gemm(int ntasks, const int64_t* c_ptr, const int32_t* ldc, cons
  * test and by bench.py's HBM probe; inside dmrg_rdm12 the same kernel serves the operator classes with nc <= 8. */
 int dmrg_stack_dots(const double* S, int64_t lds, int nrows, const double* M, int64_t ldm, int nc, int64_t K, double* E,
                     int ldE, double* ms, void* cuda_stream);
-
-/* Device time in milliseconds (CUDA events on the call's stream around the kernel launch only, descriptor upload
- * excluded) of the most recent dmrg_grouped_gemm call in this process. */
-double dmrg_last_gemm_ms(void);
-
-/* FP64 ceiling probe for the roofline denominator (SURVEY.md 8(d) D2 asks for a DMMA and a DFMA
- * issue-rate microbenchmark and the cuBLAS DGEMM figure measured on the same box).  kind 0: register-resident
- * DMMA.8x8x4 loop; 1: register-resident DFMA loop; 2: the DMMA loop fed from shared memory with the GEMM kernel's
- * fragment pattern; 3: cublasDgemm size^3.  iters: inner iterations (kinds 0-2) or DGEMM calls per timing (kind 3);
- * ctas_per_sm: resident 4-warp CTAs per SM (kinds 0-2).  Best of `reps` launches timed with CUDA events on
- * `cuda_stream`; *tflops and *ms are HOST outputs.  Not part of the product path. */
-int dmrg_fp64_probe(int kind, int iters, int ctas_per_sm, int size, int reps, double* tflops, double* ms,
-                    void* cuda_stream);
 
 #ifdef __cplusplus
 }

@@ -59,14 +59,12 @@ class dmrg_sweep_result(C.Structure):
 EXPORTS = ["dmrg_default_options", "dmrg_create", "dmrg_destroy", "dmrg_last_error", "dmrg_mps_import",
            "dmrg_mps_export", "dmrg_prepare_bond", "dmrg_heff_layout", "dmrg_heff_apply", "dmrg_heff_diag",
            "dmrg_heff_stats", "dmrg_sweep", "dmrg_sweep_stats", "dmrg_rdm12", "dmrg_rdm_stats", "dmrg_launch_count", "dmrg_flops_total", "dmrg_device_bytes",
-           "dmrg_grouped_gemm", "dmrg_stack_dots", "dmrg_last_gemm_ms", "dmrg_fp64_probe"]
+           "dmrg_grouped_gemm", "dmrg_stack_dots"]
 
 lib.dmrg_last_error.restype = C.c_char_p
 lib.dmrg_last_error.argtypes = [C.c_void_p]
 lib.dmrg_launch_count.restype = C.c_int64
 lib.dmrg_launch_count.argtypes = [C.c_void_p]
-lib.dmrg_last_gemm_ms.restype = C.c_double
-lib.dmrg_last_gemm_ms.argtypes = []
 lib.dmrg_flops_total.restype = C.c_double
 lib.dmrg_flops_total.argtypes = [C.c_void_p]
 lib.dmrg_device_bytes.restype = C.c_int64
@@ -246,9 +244,10 @@ def dmrg_device_bytes(ctx):
     return lib.dmrg_device_bytes(ctx)
 
 
-def dmrg_grouped_gemm(tasks, segs, stream=None):
+def dmrg_grouped_gemm(tasks, segs, stream=None, generic=False):
     """Kernel-level entry for the unit parity tests.  tasks: list of dict(C=ptr, ldc, M, N, seg_begin, seg_count,
-    flags); segs: list of dict(A=ptr, B=ptr, lda, ldb, K, flags, alpha); pointers are device addresses (ints)."""
+    flags); segs: list of dict(A=ptr, B=ptr, lda, ldb, K, flags, alpha); pointers are device addresses (ints).
+    generic: force the cp.async kernel.  Returns the device milliseconds of the kernel launch."""
     nt, ns = len(tasks), len(segs)
     i64 = lambda key, src: np.array([s[key] for s in src], dtype=np.int64)
     i32 = lambda key, src: np.array([s[key] for s in src], dtype=np.int32)
@@ -256,26 +255,32 @@ def dmrg_grouped_gemm(tasks, segs, stream=None):
             i32("seg_count", tasks), i32("flags", tasks)]
     sarr = [i64("A", segs), i64("B", segs), i32("lda", segs), i32("ldb", segs), i32("K", segs), i32("flags", segs),
             np.array([s["alpha"] for s in segs], dtype=np.float64)]
-    rc = lib.dmrg_grouped_gemm(nt, *[_ptr(a) for a in arrs], ns, *[_ptr(a) for a in sarr],
-                               C.c_void_p(stream or 0))
+    ms = C.c_double(0.0)
+    rc = lib.dmrg_grouped_gemm(nt, *[_ptr(a) for a in arrs], ns, *[_ptr(a) for a in sarr], 1 if generic else 0,
+                               C.byref(ms), C.c_void_p(stream or 0))
     if rc != 0:
         raise DmrgError(rc, "dmrg_grouped_gemm failed")
-    return rc
+    return ms.value
+
+
+_bench_lib = None
 
 
 def dmrg_fp64_probe(kind, iters=20000, ctas_per_sm=3, size=8192, reps=3, stream=None):
-    """FP64 ceiling probe (kind 0 DMMA, 1 DFMA, 2 DMMA fed by LDS, 3 cuBLAS DGEMM size^3): dict(tflops, ms)."""
+    """FP64 ceiling probe of the measurement-only library libdmrg_b200_bench.so (include/dmrg_b200_bench.h; kind 0 DMMA,
+    1 DFMA, 2 DMMA fed by LDS, 3 cuBLAS DGEMM size^3): dict(tflops, ms).  Not part of the product library."""
+    global _bench_lib
+    if _bench_lib is None:
+        path = os.path.join(_HERE, "libdmrg_b200_bench.so")
+        if not os.path.exists(path):
+            raise ImportError(path + " not found: run __graft_entry__.build()")
+        _bench_lib = C.CDLL(path)
     tf, ms = C.c_double(0.0), C.c_double(0.0)
-    rc = lib.dmrg_fp64_probe(int(kind), int(iters), int(ctas_per_sm), int(size), int(reps), C.byref(tf), C.byref(ms),
-                             C.c_void_p(stream or 0))
+    rc = _bench_lib.dmrg_bench_fp64_probe(int(kind), int(iters), int(ctas_per_sm), int(size), int(reps), C.byref(tf),
+                                          C.byref(ms), C.c_void_p(stream or 0))
     if rc != 0:
-        raise DmrgError(rc, "dmrg_fp64_probe failed")
+        raise DmrgError(rc, "dmrg_bench_fp64_probe failed")
     return {"tflops": tf.value, "ms": ms.value}
-
-
-def dmrg_last_gemm_ms():
-    """Device milliseconds of the kernel launched by the most recent dmrg_grouped_gemm call."""
-    return float(lib.dmrg_last_gemm_ms())
 
 
 def dmrg_flops_total(ctx):

@@ -452,17 +452,16 @@ int dmrg_stack_dots(const double* S, int64_t lds, int nrows, const double* M, in
     return (err == cudaSuccess && cudaGetLastError() == cudaSuccess) ? DMRG_OK : DMRG_ECUDA;
 }
 
-static double g_last_gemm_ms = 0.0;
-double dmrg_last_gemm_ms(void) { return g_last_gemm_ms; }
-
 int dmrg_grouped_gemm(int ntasks, const int64_t* c_ptr, const int32_t* ldc, const int32_t* m, const int32_t* n,
                       const int32_t* seg_begin, const int32_t* seg_count, const int32_t* task_flags, int nsegs,
                       const int64_t* a_ptr, const int64_t* b_ptr, const int32_t* lda, const int32_t* ldb,
-                      const int32_t* kk, const int32_t* seg_flags, const double* alpha, void* cuda_stream) {
+                      const int32_t* kk, const int32_t* seg_flags, const double* alpha, int generic_kernel,
+                      double* kernel_ms, void* cuda_stream) {
     if (ntasks < 0 || nsegs < 0) return DMRG_EINVAL;
     try {
         Engine tmp;                                            // only the stream and the launch counter are used
         tmp.stream = (cudaStream_t)cuda_stream;
+        tmp.force_generic_gemm = generic_kernel != 0;
         GemmBatch b;
         for (int t = 0; t < ntasks; ++t) {
             if (seg_begin[t] < 0 || seg_count[t] < 0 || seg_begin[t] + seg_count[t] > nsegs) return DMRG_EINVAL;
@@ -483,22 +482,13 @@ int dmrg_grouped_gemm(int ntasks, const int64_t* c_ptr, const int32_t* ldc, cons
             cuda_check(cudaStreamSynchronize(tmp.stream), "grouped GEMM");
             float ms = 0.f;
             cudaEventElapsedTime(&ms, e0, e1);
-            g_last_gemm_ms = ms;
+            if (kernel_ms) *kernel_ms = ms;
             cudaEventDestroy(e0);
             cudaEventDestroy(e1);
         }
     } catch (const Error& e) { return e.code; }
     catch (...) { return DMRG_ECUDA; }
     return DMRG_OK;
-}
-
-int dmrg_fp64_probe(int kind, int iters, int ctas_per_sm, int size, int reps, double* tflops, double* ms,
-                    void* cuda_stream) {
-    if (kind < 0 || kind > 3 || iters < 1 || reps < 1 || !tflops || !ms) return DMRG_EINVAL;
-    if (kind < 3 && (ctas_per_sm < 1 || ctas_per_sm > 16)) return DMRG_EINVAL;
-    if (kind == 3 && (size < 1 || size > 32768)) return DMRG_EINVAL;
-    const int rc = fp64_probe(kind, iters, ctas_per_sm, size, reps, tflops, ms, (cudaStream_t)cuda_stream);
-    return rc == 0 ? DMRG_OK : (rc == -3 ? DMRG_ENOMEM : DMRG_ECUDA);
 }
 
 }  // extern "C"

@@ -1,16 +1,19 @@
 // FP64 ceiling probes for the roofline denominator:
 // register-resident DMMA.8x8x4 and DFMA issue-rate loops, the same DMMA loop fed from shared memory with the
-// fragment pattern of the grouped GEMM kernel, and cuBLAS DGEMM on a square problem.  Not on the product path.
+// fragment pattern of the grouped GEMM kernel, and cuBLAS DGEMM on a square problem.  Measurement only: built into the
+// separate library libdmrg_b200_bench.so (include/dmrg_b200_bench.h); the product library neither contains nor links it.
 #include <cublas_v2.h>
 #include <cuda_runtime.h>
 
 #include <cstdint>
 
-#include "kernels.hpp"
+#include "../../../include/dmrg_b200_bench.h"
 
 namespace dmrg {
 
 namespace {
+
+constexpr int GEMM_BM = 64, GEMM_BN = 64, GEMM_BK = 16;   // tile shape of the product GEMM kernel (stated here: no shared header)
 
 __device__ __forceinline__ void dmma_p(double& d0, double& d1, double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
@@ -86,7 +89,7 @@ __global__ void __launch_bounds__(128) probe_dmma_lds(int iters, double* sink) {
 
 // kind 0: DMMA registers only; 1: DFMA; 2: DMMA fed by LDS; 3: cuBLAS DGEMM n x n x n (iters = repetitions, n = size)
 // ctas_per_sm resident CTAs of 4 warps.  Returns 0 on success; tflops and ms of the best of `reps` timed launches.
-int fp64_probe(int kind, int iters, int ctas_per_sm, int size, int reps, double* tflops, double* ms, cudaStream_t st) {
+static int fp64_probe(int kind, int iters, int ctas_per_sm, int size, int reps, double* tflops, double* ms, cudaStream_t st) {
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -145,3 +148,12 @@ int fp64_probe(int kind, int iters, int ctas_per_sm, int size, int reps, double*
 }
 
 }  // namespace dmrg
+
+extern "C" int dmrg_bench_fp64_probe(int kind, int iters, int ctas_per_sm, int size, int reps, double* tflops, double* ms,
+                                     void* cuda_stream) {
+    if (kind < 0 || kind > 3 || iters < 1 || reps < 1 || !tflops || !ms) return -1;
+    if (kind < 3 && (ctas_per_sm < 1 || ctas_per_sm > 16)) return -1;
+    if (kind == 3 && (size < 1 || size > 32768)) return -1;
+    const int rc = dmrg::fp64_probe(kind, iters, ctas_per_sm, size, reps, tflops, ms, (cudaStream_t)cuda_stream);
+    return rc == 0 ? 0 : (rc == -3 ? -3 : -4);
+}

@@ -1,5 +1,5 @@
 // Launchers of the sm_100a CUDA kernels (the only place tensor arithmetic happens).  Implemented in seg_gemm_tma.cu,
-// seg_gemm.cu, vec_kernels.cu, linalg.cu and probe.cu (the integer block-map kernels are in heff_maps.cu / maps.hpp).  All pointers are device pointers unless a name ends in _host.
+// seg_gemm.cu, vec_kernels.cu and linalg.cu (the integer block-map kernels are in heff_maps.cu / maps.hpp).  All pointers are device pointers unless a name ends in _host.
 #pragma once
 #include <cuda_runtime_api.h>
 
@@ -86,8 +86,5 @@ struct SvdWork;
 SvdWork* svd_create(cudaStream_t st, bool jacobi);   // jacobi: gesvdj (gesvd fallback), else gesvd
 void svd_destroy(SvdWork* w);
 void svd_rowmajor(SvdWork* w, double* A, int m, int n, double* U, double* S, double* Vt, cudaStream_t st);
-
-// ---- FP64 ceiling probes (probe.cu; measurement only) -----------------------------------------------------------------
-int fp64_probe(int kind, int iters, int ctas_per_sm, int size, int reps, double* tflops, double* ms, cudaStream_t st);
 
 }  // namespace dmrg

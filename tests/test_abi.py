@@ -6,8 +6,8 @@ import re
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def declared_symbols():
-    src = open(os.path.join(ROOT, "include", "dmrg_b200.h")).read()
+def declared_symbols(header="dmrg_b200.h"):
+    src = open(os.path.join(ROOT, "include", header)).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(dmrg_[a-z0-9_]+)\s*\(", src)))
 
@@ -19,6 +19,11 @@ def test_library_exports_every_declared_symbol(lib):
     for n in names:
         assert hasattr(dll, n), "missing export " + n
     assert sorted(lib.binding.EXPORTS) == names
+    # the measurement-only companion library: its own header, its own .so; the product library carries none of it
+    bench = ctypes.CDLL(os.path.join(os.path.dirname(lib.binding.LIB_PATH), "libdmrg_b200_bench.so"))
+    for n in declared_symbols("dmrg_b200_bench.h"):
+        assert hasattr(bench, n), "missing export " + n
+        assert not hasattr(dll, n)
 
 
 def test_default_options_and_argument_errors_need_no_gpu(lib):

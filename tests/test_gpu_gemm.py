@@ -6,12 +6,12 @@ import pytest
 pytestmark = pytest.mark.gpu
 
 
-def _case(lib, rng, shapes, accumulate):
+def _case(lib, rng, shapes, accumulate, generic=False, aligned=False):
     import torch
     dev = torch.device("cuda:0")
     tasks, segs, keep, expect = [], [], [], []
     for (M, N, ks) in shapes:
-        ldc = N + int(rng.integers(0, 3))
+        ldc = N + (0 if aligned else int(rng.integers(0, 3)))
         c0 = rng.normal(size=(M, ldc))
         Cd = torch.tensor(c0, device=dev)
         keep.append(Cd)
@@ -29,6 +29,8 @@ def _case(lib, rng, shapes, accumulate):
                 ref += alpha * a[:, :N]
                 continue
             pa, pb = int(rng.integers(0, 2)), int(rng.integers(0, 2))
+            if aligned:                                           # even leading dimensions covering pad2(extent): bulk-copy kernel eligible
+                pa, pb = (M if (fl & 1) else K) % 2 + 2, (K if (fl & 2) else N) % 2 + 2
             a = rng.normal(size=(K, M + pa)) if (fl & 1) else rng.normal(size=(M, K + pa))
             b = rng.normal(size=(N, K + pb)) if (fl & 2) else rng.normal(size=(K, N + pb))
             Ad, Bd = torch.tensor(a, device=dev), torch.tensor(b, device=dev)
@@ -41,8 +43,9 @@ def _case(lib, rng, shapes, accumulate):
                           flags=1 if accumulate else 0))
         expect.append((Cd, ref, c0, N))
     torch.cuda.synchronize()
-    lib.dmrg_grouped_gemm(tasks, segs, torch.cuda.current_stream().cuda_stream)
+    ms = lib.dmrg_grouped_gemm(tasks, segs, torch.cuda.current_stream().cuda_stream, generic=generic)
     torch.cuda.synchronize()
+    assert ms > 0.0
     for (Cd, ref, c0, N) in expect:
         got = Cd.cpu().numpy()
         scale = max(1.0, np.abs(ref).max())
@@ -64,9 +67,19 @@ def test_grouped_gemm_many_segments_spanning_tiles(lib):
     _case(lib, rng, shapes, False)
 
 
+@pytest.mark.parametrize("generic", [False, True])
+def test_grouped_gemm_aligned_operands_both_kernels(lib, generic):
+    """16-byte aligned operands with even leading dimensions: the bulk-copy (TMA engine) kernel, and the cp.async kernel
+    forced on the same problem."""
+    rng = np.random.default_rng(23)
+    shapes = [(64, 64, [16, 48]), (150, 170, [int(k) for k in rng.integers(1, 90, size=12)]), (9, 300, [77, 0, 5]), (257, 129, [300, 7])]
+    _case(lib, rng, shapes, False, generic=generic, aligned=True)
+    _case(lib, rng, shapes, True, generic=generic, aligned=True)
+
+
 def test_probe_and_counters(lib):
-    """dmrg_fp64_probe returns plausible ceilings (DMMA within 50-110 % of the nominal 37.2 TFLOP/s of a B200),
-    dmrg_last_gemm_ms times the kernel of the last dmrg_grouped_gemm call, dmrg_flops_total counts unpadded flops."""
+    """The bench-only probe library returns plausible ceilings (DMMA within 50-110 % of the nominal 37.2 TFLOP/s of a
+    B200); dmrg_flops_total counts unpadded flops."""
     import torch
     r = lib.dmrg_fp64_probe(0, iters=4000, ctas_per_sm=3, reps=2)
     assert 0.5 * 37.2 <= r["tflops"] <= 1.1 * 37.2 and r["ms"] > 0
@@ -74,9 +87,6 @@ def test_probe_and_counters(lib):
     assert 5.0 <= r1["tflops"] <= 1.1 * 37.2
     with pytest.raises(lib.binding.DmrgError):
         lib.dmrg_fp64_probe(7)
-    rng = np.random.default_rng(3)
-    _case(lib, rng, [(128, 96, [64, 32])], False)
-    assert lib.dmrg_last_gemm_ms() > 0.0
     from synth import random_dense, random_mps, mps_to_blob_arrays
     k, n = 6, 6
     h, eri = random_dense(k, 1)
