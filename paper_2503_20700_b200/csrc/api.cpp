@@ -126,6 +126,7 @@ int dmrg_create(dmrg_ctx** out, int k, int n_elec, int two_sz, const double* h, 
         eng.ham.h.assign(h, h + (size_t)k * k);
         eng.ham.eri.assign(eri, eri + (size_t)k * k * k * k);
         eng.svd = svd_create(eng.stream, eng.opt.svd_qr == 0);
+        eng.red_scratch.alloc((size_t)multi_dot_scratch());
         { const char* g = std::getenv("DMRG_B200_TRACE"); eng.trace = g && g[0] == '1'; }   // diagnostics only: per-launch times on stderr
     } catch (...) {
         delete ctx;
@@ -141,8 +142,11 @@ int dmrg_destroy(dmrg_ctx* ctx) {
     cudaSetDevice(eng.opt.device_id);
     eng.invalidate();
     eng.host_pool.clear();
+    eng.red_scratch.release();
     eng.mps.sites.clear();
     if (eng.svd) svd_destroy(eng.svd);
+    for (SvdWork* w : eng.svd_pool) svd_destroy(w);
+    for (cudaStream_t ts : eng.svd_streams) cudaStreamDestroy(ts);
     if (eng.stream) cudaStreamDestroy(eng.stream);
     if (eng.stream2) cudaStreamDestroy(eng.stream2);
     if (eng.copy_stream) cudaStreamDestroy(eng.copy_stream);

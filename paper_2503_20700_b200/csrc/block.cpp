@@ -1,7 +1,9 @@
 // Device-resident block operators: storage, launch-descriptor plumbing, linear combinations, blocking (grow).
 #include <algorithm>
 #include <cassert>
+#include <cmath>
 #include <cstdio>
+#include <mutex>
 
 #include "core.hpp"
 
@@ -12,6 +14,7 @@ namespace dmrg {
 // ---------------------------------------------------------------------------------------------------------------
 int64_t g_device_bytes = 0;
 static std::unordered_map<void*, size_t> g_sizes;
+static std::mutex g_alloc_mutex;                           // allocations also come from the host threads of split_theta
 
 void cuda_check(cudaError_t e, const char* what) {
     if (e != cudaSuccess) throw Error(-4, std::string(what) + ": " + cudaGetErrorString(e));
@@ -22,14 +25,18 @@ void* dev_alloc(size_t bytes) {
     cudaError_t e = cudaMalloc(&p, bytes);
     if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); throw Error(-3, "out of device memory"); }
     cuda_check(e, "cudaMalloc");
+    std::lock_guard<std::mutex> lock(g_alloc_mutex);
     g_sizes[p] = bytes;
     g_device_bytes += (int64_t)bytes;
     return p;
 }
 void dev_free(void* p) {
     if (!p) return;
-    auto it = g_sizes.find(p);
-    if (it != g_sizes.end()) { g_device_bytes -= (int64_t)it->second; g_sizes.erase(it); }
+    {
+        std::lock_guard<std::mutex> lock(g_alloc_mutex);
+        auto it = g_sizes.find(p);
+        if (it != g_sizes.end()) { g_device_bytes -= (int64_t)it->second; g_sizes.erase(it); }
+    }
     cudaFree(p);
 }
 
@@ -80,68 +87,87 @@ void GemmBatch::add_seg(int task, const double* A, int lda, const double* B, int
 
 void finalize(GemmBatch& b, GemmLaunch& out, Engine& eng) {
     const int nt = (int)b.tasks.size();
+    const size_t ns = b.segs.size();
     // Order within a task: GEMM segments first, sorted by alpha (stable), identity-B segments last.  Empty products
     // (K <= 0 or alpha == 0) are dropped.  Equal alphas adjacent let the bulk-copy kernel keep its accumulators in
     // units of the current alpha and rescale them only when alpha changes (no per-fragment multiply in the main loop).
-    std::vector<std::vector<int>> by_task(nt);
-    for (size_t j = 0; j < b.segs.size(); ++j) {
+    // Counting sort of the segments by task (stable), then one small sort per task - tasks in parallel on the host.
+    std::vector<int> off((size_t)nt + 1, 0);
+    for (size_t j = 0; j < ns; ++j) {
         const Seg& sg = b.segs[j];
         if (!(sg.flags & SEG_IDENT_B) && (sg.K <= 0 || sg.alpha == 0.0)) continue;
-        by_task[b.seg_task[j]].push_back((int)j);
+        off[(size_t)b.seg_task[j] + 1]++;
     }
-    std::vector<Seg> sorted;
-    sorted.reserve(b.segs.size());
+    for (int t = 0; t < nt; ++t) off[t + 1] += off[t];
+    std::vector<int> idx((size_t)off[nt]), fill(off.begin(), off.end() - 1);
+    for (size_t j = 0; j < ns; ++j) {
+        const Seg& sg = b.segs[j];
+        if (!(sg.flags & SEG_IDENT_B) && (sg.K <= 0 || sg.alpha == 0.0)) continue;
+        idx[(size_t)fill[b.seg_task[j]]++] = (int)j;
+    }
+    std::vector<Seg> sorted((size_t)off[nt]);
+    std::vector<double> weight(nt, 0.0);
+    std::vector<int> ntile((size_t)nt + 1, 0);
+    int aligned_i = 1;
+#pragma omp parallel for schedule(static, 256) reduction(&& : aligned_i)
     for (int t = 0; t < nt; ++t) {
-        std::vector<int>& v = by_task[t];
-        std::stable_sort(v.begin(), v.end(), [&](int x, int y) {
+        int* v0 = idx.data() + off[t];
+        int* v1 = idx.data() + off[t + 1];
+        std::stable_sort(v0, v1, [&](int x, int y) {
             const bool ix = b.segs[x].flags & SEG_IDENT_B, iy = b.segs[y].flags & SEG_IDENT_B;
             if (ix != iy) return iy;
             if (ix) return false;
             return b.segs[x].alpha < b.segs[y].alpha;
         });
-        b.tasks[t].seg_begin = (int)sorted.size();
-        b.tasks[t].seg_count = (int)v.size();
-        b.tasks[t].ngemm = 0;
-        for (int j : v) {
-            if (!(b.segs[j].flags & SEG_IDENT_B)) b.tasks[t].ngemm++;
-            sorted.push_back(b.segs[j]);
+        Task& tk = b.tasks[t];
+        tk.seg_begin = off[t];
+        tk.seg_count = off[t + 1] - off[t];
+        tk.ngemm = 0;
+        double w = 0.0;
+        bool al = true;
+        for (int* q = v0; q != v1; ++q) {
+            const Seg& sg = b.segs[*q];
+            sorted[(size_t)(q - idx.data())] = sg;
+            w += sg.K;
+            if (sg.flags & SEG_IDENT_B) continue;
+            tk.ngemm++;
+            // bulk-copy kernel: 16-byte aligned operands, even leading dimensions; a transposed / row operand is read
+            // in pieces of pad2(extent) doubles, so the leading dimension must cover them
+            if ((((uintptr_t)sg.A) & 15) || (((uintptr_t)sg.B) & 15) || (sg.lda & 1) || (sg.ldb & 1)) al = false;
+            const int needA = (sg.flags & SEG_TRANS_A) ? pad2(tk.M) : pad2(sg.K);
+            const int needB = (sg.flags & SEG_TRANS_B) ? pad2(sg.K) : pad2(tk.N);
+            if (sg.lda < needA || sg.ldb < needB) al = false;
+        }
+        weight[t] = w;
+        aligned_i = aligned_i && al;
+        if (tk.M > 0 && tk.N > 0) {
+            const int nm = (tk.M + GEMM_BM - 1) / GEMM_BM, nn = (tk.N + GEMM_BN - 1) / GEMM_BN;
+            const int pm = std::min(GEMM_BM, (((tk.M + nm - 1) / nm) + 7) & ~7), pn = std::min(GEMM_BN, (((tk.N + nn - 1) / nn) + 7) & ~7);
+            ntile[(size_t)t + 1] = ((tk.M + pm - 1) / pm) * ((tk.N + pn - 1) / pn);
         }
     }
-    bool aligned = true;
-    for (const Seg& sg : sorted) {
-        if (sg.flags & SEG_IDENT_B) continue;
-        if ((((uintptr_t)sg.A) & 15) || (((uintptr_t)sg.B) & 15) || (sg.lda & 1) || (sg.ldb & 1)) { aligned = false; break; }
-    }
-    // a transposed / row operand is read in pieces of pad2(extent) doubles: the leading dimension must cover them
-    for (int t = 0; t < nt && aligned; ++t)
-        for (int j = 0; j < b.tasks[t].ngemm; ++j) {
-            const Seg& sg = sorted[b.tasks[t].seg_begin + j];
-            const int M = b.tasks[t].M, N = b.tasks[t].N, K = sg.K;
-            const int needA = (sg.flags & SEG_TRANS_A) ? pad2(M) : pad2(K);
-            const int needB = (sg.flags & SEG_TRANS_B) ? pad2(K) : pad2(N);
-            if (sg.lda < needA || sg.ldb < needB) { aligned = false; break; }
-        }
-    out.aligned = aligned;
-    // tiles, heaviest tasks first so that the tail of the launch is made of short tiles
-    std::vector<double> weight(nt, 0.0);
-    for (int t = 0; t < nt; ++t)
-        for (int j = 0; j < b.tasks[t].seg_count; ++j) weight[t] += sorted[b.tasks[t].seg_begin + j].K;
-    // tiles, heaviest first (weight = K extent x DMMA fragments of the tile) so that the persistent kernel's dynamic
-    // tile counter ends the launch on short tiles
-    std::vector<Tile> raw;
-    std::vector<double> tw;
+    out.aligned = aligned_i != 0;
+    // tiles: even split of each extent into ceil(extent / 64) pieces rounded up to the 8-row DMMA fragment (the kernel
+    // skips fragments outside [mv x nv], so the padding waste is at the 8 level, not the 64 level); heaviest first
+    // (weight = K extent x DMMA fragments of the tile) so that the persistent kernel's dynamic tile counter ends the
+    // launch on short tiles
+    for (int t = 0; t < nt; ++t) ntile[(size_t)t + 1] += ntile[t];
+    const size_t ntl = (size_t)ntile[nt];
+    std::vector<Tile> raw(ntl);
+    std::vector<double> tw(ntl);
+#pragma omp parallel for schedule(static, 256)
     for (int t = 0; t < nt; ++t) {
         const Task& tk = b.tasks[t];
         if (tk.M <= 0 || tk.N <= 0) continue;
-        // even split of each extent into ceil(extent / 64) pieces rounded up to the 8-row DMMA fragment: the kernel
-        // skips fragments outside [mv x nv], so the padding waste is at the 8 level, not the 64 level
         const int nm = (tk.M + GEMM_BM - 1) / GEMM_BM, nn = (tk.N + GEMM_BN - 1) / GEMM_BN;
         const int pm = std::min(GEMM_BM, (((tk.M + nm - 1) / nm) + 7) & ~7), pn = std::min(GEMM_BN, (((tk.N + nn - 1) / nn) + 7) & ~7);
+        size_t q = (size_t)ntile[t];
         for (int m0 = 0; m0 < tk.M; m0 += pm)
             for (int n0 = 0; n0 < tk.N; n0 += pn) {
                 const int mv = std::min(pm, tk.M - m0), nv = std::min(pn, tk.N - n0);
-                raw.push_back({t, m0, n0, mv, nv});
-                tw.push_back((weight[t] + 16.0) * ((mv + 7) / 8) * ((nv + 7) / 8));
+                raw[q] = {t, m0, n0, mv, nv};
+                tw[q] = (weight[t] + 16.0) * ((mv + 7) / 8) * ((nv + 7) / 8);
+                ++q;
             }
     }
     if (eng.trace) {                                           // flop and stage histogram by fragments of the busiest warp
@@ -157,11 +183,20 @@ void finalize(GemmBatch& b, GemmLaunch& out, Engine& eng) {
             if (hs[c] > 0) std::fprintf(stderr, " %d:%.1f/%.1f", c, 100.0 * hf[c] / tf, 100.0 * hs[c] / ts);
         std::fprintf(stderr, "\n");
     }
-    std::vector<int> order(raw.size());
-    for (size_t j = 0; j < raw.size(); ++j) order[j] = (int)j;
-    std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return tw[x] > tw[y]; });
-    std::vector<Tile> tiles(raw.size());
-    for (size_t j = 0; j < raw.size(); ++j) tiles[j] = raw[order[j]];
+    // stable counting sort by weight, heaviest first, on 1/16-octave buckets (the order only balances the load: results do
+    // not depend on it, every tile is owned by one CTA and its summation order is the segment order)
+    constexpr int NB = 1024;
+    std::vector<int> bucket(ntl);
+    std::vector<size_t> hist(NB + 1, 0);
+    for (size_t j = 0; j < ntl; ++j) {
+        int q = (int)(std::log2(std::max(tw[j], 1.0)) * 16.0);
+        q = NB - 1 - std::min(NB - 1, std::max(0, q));          // heavy tiles -> low bucket
+        bucket[j] = q;
+        hist[(size_t)q + 1]++;
+    }
+    for (int q = 0; q < NB; ++q) hist[(size_t)q + 1] += hist[q];
+    std::vector<Tile> tiles(ntl);
+    for (size_t j = 0; j < ntl; ++j) tiles[hist[bucket[j]]++] = raw[j];
     out.tasks.upload(b.tasks, eng.stream);
     out.segs.upload(sorted, eng.stream);
     out.tiles.upload(tiles, eng.stream);

@@ -251,6 +251,10 @@ struct Engine {
     double flops_total = 0;                       // unpadded flops of every grouped-GEMM launch since creation
     std::string last_error;
     SvdWork* svd = nullptr;
+    DevVec<double> red_scratch;                   // partial sums of the two-stage reductions (per context)
+    std::vector<SvdWork*> svd_pool;               // extra cuSOLVER handles on their own streams: sector SVDs run concurrently
+    std::vector<cudaStream_t> svd_streams;
+    void ensure_svd_pool(int n);
     double rdm_seconds = 0, rdm_bytes = 0, rdm_flops = 0, rdm_host_seconds = 0, rdm_grow_seconds = 0, rdm_gemm_ms = 0;
     double rdm_stream_bytes = 0;                  // bytes of the launches of the HBM-bound streaming kernel alone
     double t_plan = 0, t_davidson = 0, t_split = 0, t_grow = 0, t_matvec = 0;   // phase seconds of the last sweep

@@ -89,24 +89,23 @@ void make_temps(const Ham& ham, Block& X, const Dot& dot, const std::vector<int>
 // ---------------------------------------------------------------------------------------------------------------
 struct NewOp { Label label; Expr expr; };
 
-static void rotate_batch(Block& X, const Dot& dot, const SiteTensor& tensor, Block& nb, const std::vector<NewOp>& list,
-                         bool temp, Engine& eng) {
-    std::vector<Label> labels;
-    for (const NewOp& o : list) labels.push_back(o.label);
-    nb.allocate(labels, temp);
+// Descriptors of ONE new operator, built by one host thread: T pointers are relative to offset 0 of the workspace and
+// task indices are local; merge() below rebases both into the launch-wide batches.
+struct OpPlan {
+    GemmBatch p1, p2;
+    std::vector<int> tsegs;                        // phase-2 segments whose B operand is a workspace buffer
+    int64_t used = 0;
+};
+
+static void plan_op(Block& X, const Dot& dot, const SiteTensor& tensor, Block& nb, const NewOp& no, int64_t cap,
+                    OpPlan& out) {
+    double* const tbase = nullptr;                         // workspace addresses are offsets until merge() rebases them
     const bool left = X.side == 'L';
     const char* chain = left ? "Ld" : "dR";
     const int nnew = (int)nb.basis.size();
-    const int64_t cap = eng.t_capacity();
-    DevVec<double> tmp;
-    tmp.alloc((size_t)cap);
-    GemmBatch p1, p2;
-    int64_t used = 0;
-    auto flush = [&]() {
-        run_once(p1, eng);
-        run_once(p2, eng);
-        used = 0;
-    };
+    GemmBatch& p1 = out.p1;
+    GemmBatch& p2 = out.p2;
+    int64_t& used = out.used;
     // new-basis sector reached from X-sector i by adding (left) / removing (right) site state s
     auto new_sector = [&](int i, int s) {
         const Sector& q = X.basis[i];
@@ -117,82 +116,159 @@ static void rotate_batch(Block& X, const Dot& dot, const SiteTensor& tensor, Blo
         if (newsec < 0) return nullptr;
         return left ? tensor.get(xsec, s) : tensor.get(newsec, s);
     };
-    for (const NewOp& no : list) {
-        const OpRef& ref = nb.get(no.label);
-        const OpClass& nc = nb.classes[ref.cls];
-        std::vector<int> p2task(nnew, -1);
-        auto out_task = [&](int mi) {
-            if (p2task[mi] < 0)
-                p2task[mi] = p2.add_task(ref.ptr + nc.off[mi], pad2(nb.basis[mi].d), nb.basis[nc.out[mi]].d,
-                                         nb.basis[mi].d, 0);
-            return p2task[mi];
-        };
-        for (int mi = 0; mi < nnew; ++mi)
-            if (nc.out[mi] >= 0) out_task(mi);                 // every block is written (zero if nothing feeds it)
-        std::map<int64_t, std::pair<int, double*>> tmps;       // (o, so, mi) -> (phase-1 task, buffer)
-        for (const Term& term : no.expr) {
-            const NTerm nt = normalise(term, chain, dot);
-            const bool has_op = left ? nt.hasL : nt.hasR;
-            const Label& lab = left ? nt.L : nt.R;
-            const bool tr = left ? nt.transL : nt.transR;
-            const OpRef* op = has_op ? &X.get(lab) : nullptr;
-            const int po = has_op ? KIND_PAR[lab.kind] : 0;
-            const int pm = dot.parity(nt.dm);
-            for (int so = 0; so < 4; ++so)
-                for (int si = 0; si < 4; ++si) {
-                    const double dmv = nt.dm(so, si);
-                    if (dmv == 0.0) continue;
-                    for (int i = 0; i < (int)X.basis.size(); ++i) {
-                        OpBlockView v;
-                        int o = i;
-                        if (op) { if (!op_block(X, *op, tr, i, v)) continue; o = v.out; }
-                        const int mi = new_sector(i, si), mo = new_sector(o, so);
-                        const SiteTensor::Blk* ti = tensor_block(i, si, mi);
-                        const SiteTensor::Blk* to = tensor_block(o, so, mo);
-                        if (!ti || !to) continue;
-                        if (nc.out[mi] != mo) throw std::logic_error("rotate: quantum numbers do not close");
-                        const double sgn = left ? ((pm && (X.basis[i].n & 1)) ? -1.0 : 1.0)
-                                                : ((po && (SITE_QN[si] & 1)) ? -1.0 : 1.0);
-                        const double alpha = nt.coef * dmv * sgn;
-                        const int di = X.basis[i].d, dO = X.basis[o].d, dmi = nb.basis[mi].d;
-                        if (!op) {                             // identity block factor: straight into phase 2
-                            if (left) p2.add_seg(out_task(mi), to->ptr, to->ld, ti->ptr, ti->ld, di, SEG_TRANS_A, alpha);
-                            else      p2.add_seg(out_task(mi), to->ptr, to->ld, ti->ptr, ti->ld, di, SEG_TRANS_B, alpha);
-                            continue;
-                        }
-                        const int64_t key = ((int64_t)o * 4 + so) * nnew + mi;
-                        auto it = tmps.find(key);
-                        if (it == tmps.end()) {
-                            const int64_t sz = (int64_t)dO * pad2(dmi);
-                            if (used + sz > cap) throw Error(-3, "renormalisation workspace too small");
-                            double* buf = tmp.p + used;
-                            used += sz;
-                            const int t1 = p1.add_task(buf, pad2(dmi), dO, dmi, 0);
-                            it = tmps.emplace(key, std::make_pair(t1, buf)).first;
-                            // phase 2: out[mo <- mi] += to^T tmp (left) / to tmp (right)
-                            if (left) p2.add_seg(out_task(mi), to->ptr, to->ld, buf, pad2(dmi), dO, SEG_TRANS_A, 1.0);
-                            else      p2.add_seg(out_task(mi), to->ptr, to->ld, buf, pad2(dmi), dO, 0, 1.0);
-                        }
-                        int fl = v.trans ? SEG_TRANS_A : 0;
-                        if (!left) fl |= SEG_TRANS_B;          // ti stored [d_m x d_i]
-                        p1.add_seg(it->second.first, v.ptr, v.ld, ti->ptr, ti->ld, di, fl, alpha);
+    const OpRef& ref = nb.get(no.label);
+    const OpClass& nc = nb.classes[ref.cls];
+    std::vector<int> p2task(nnew, -1);
+    auto out_task = [&](int mi) {
+        if (p2task[mi] < 0)
+            p2task[mi] = p2.add_task(ref.ptr + nc.off[mi], pad2(nb.basis[mi].d), nb.basis[nc.out[mi]].d,
+                                     nb.basis[mi].d, 0);
+        return p2task[mi];
+    };
+    for (int mi = 0; mi < nnew; ++mi)
+        if (nc.out[mi] >= 0) out_task(mi);                 // every block is written (zero if nothing feeds it)
+    std::unordered_map<int64_t, std::pair<int, double*>> tmps;   // (o, so, mi) -> (phase-1 task, buffer)
+    for (const Term& term : no.expr) {
+        const NTerm nt = normalise(term, chain, dot);
+        const bool has_op = left ? nt.hasL : nt.hasR;
+        const Label& lab = left ? nt.L : nt.R;
+        const bool tr = left ? nt.transL : nt.transR;
+        const OpRef* op = has_op ? &X.get(lab) : nullptr;
+        const int po = has_op ? KIND_PAR[lab.kind] : 0;
+        const int pm = dot.parity(nt.dm);
+        for (int so = 0; so < 4; ++so)
+            for (int si = 0; si < 4; ++si) {
+                const double dmv = nt.dm(so, si);
+                if (dmv == 0.0) continue;
+                for (int i = 0; i < (int)X.basis.size(); ++i) {
+                    OpBlockView v;
+                    int o = i;
+                    if (op) { if (!op_block(X, *op, tr, i, v)) continue; o = v.out; }
+                    const int mi = new_sector(i, si), mo = new_sector(o, so);
+                    const SiteTensor::Blk* ti = tensor_block(i, si, mi);
+                    const SiteTensor::Blk* to = tensor_block(o, so, mo);
+                    if (!ti || !to) continue;
+                    if (nc.out[mi] != mo) throw std::logic_error("rotate: quantum numbers do not close");
+                    const double sgn = left ? ((pm && (X.basis[i].n & 1)) ? -1.0 : 1.0)
+                                            : ((po && (SITE_QN[si] & 1)) ? -1.0 : 1.0);
+                    const double alpha = nt.coef * dmv * sgn;
+                    const int di = X.basis[i].d, dO = X.basis[o].d, dmi = nb.basis[mi].d;
+                    if (!op) {                             // identity block factor: straight into phase 2
+                        if (left) p2.add_seg(out_task(mi), to->ptr, to->ld, ti->ptr, ti->ld, di, SEG_TRANS_A, alpha);
+                        else      p2.add_seg(out_task(mi), to->ptr, to->ld, ti->ptr, ti->ld, di, SEG_TRANS_B, alpha);
+                        continue;
                     }
+                    const int64_t key = ((int64_t)o * 4 + so) * nnew + mi;
+                    auto it = tmps.find(key);
+                    if (it == tmps.end()) {
+                        const int64_t sz = (int64_t)dO * pad2(dmi);
+                        if (used + sz > cap) throw Error(-3, "renormalisation workspace too small");
+                        double* buf = tbase + used;
+                        used += sz;
+                        const int t1 = p1.add_task(buf, pad2(dmi), dO, dmi, 0);
+                        it = tmps.emplace(key, std::make_pair(t1, buf)).first;
+                        // phase 2: out[mo <- mi] += to^T tmp (left) / to tmp (right)
+                        if (left) p2.add_seg(out_task(mi), to->ptr, to->ld, buf, pad2(dmi), dO, SEG_TRANS_A, 1.0);
+                        else      p2.add_seg(out_task(mi), to->ptr, to->ld, buf, pad2(dmi), dO, 0, 1.0);
+                        out.tsegs.push_back((int)p2.segs.size() - 1);
+                    }
+                    int fl = v.trans ? SEG_TRANS_A : 0;
+                    if (!left) fl |= SEG_TRANS_B;          // ti stored [d_m x d_i]
+                    p1.add_seg(it->second.first, v.ptr, v.ld, ti->ptr, ti->ld, di, fl, alpha);
                 }
+            }
+    }
+}
+
+// append the plan of one operator to the launch-wide batches: task indices shifted, workspace offsets turned into
+// addresses at `base`
+static void merge(GemmBatch& p1, GemmBatch& p2, const OpPlan& pl, double* base) {
+    const int t1 = (int)p1.tasks.size(), t2 = (int)p2.tasks.size();
+    const size_t s2 = p2.segs.size();
+    for (Task t : pl.p1.tasks) { t.C = base + (t.C - (double*)nullptr); p1.tasks.push_back(t); }
+    p1.segs.insert(p1.segs.end(), pl.p1.segs.begin(), pl.p1.segs.end());
+    for (int t : pl.p1.seg_task) p1.seg_task.push_back(t1 + t);
+    p1.flops += pl.p1.flops;
+    p2.tasks.insert(p2.tasks.end(), pl.p2.tasks.begin(), pl.p2.tasks.end());
+    p2.segs.insert(p2.segs.end(), pl.p2.segs.begin(), pl.p2.segs.end());
+    for (int j : pl.tsegs) p2.segs[s2 + j].B = base + (p2.segs[s2 + j].B - (const double*)nullptr);
+    for (int t : pl.p2.seg_task) p2.seg_task.push_back(t2 + t);
+    p2.flops += pl.p2.flops;
+}
+
+static void rotate_batch(Block& X, const Dot& dot, const SiteTensor& tensor, Block& nb, const std::vector<NewOp>& list,
+                         bool temp, Engine& eng) {
+    std::vector<Label> labels;
+    for (const NewOp& o : list) labels.push_back(o.label);
+    nb.allocate(labels, temp);
+    const int64_t cap = eng.t_capacity();
+    // The integer descriptors of the new operators are independent of each other: host threads plan them (workspace
+    // addresses as offsets from zero), then the plans are appended in list order, so the launches do not depend on the
+    // number of threads.  The workspace is sized by what the plans need (at most `cap`: then in several flushes).
+    std::vector<OpPlan> plans(list.size());
+    std::string err;
+    int err_code = 0;
+#pragma omp parallel for schedule(dynamic, 4)
+    for (long j = 0; j < (long)list.size(); ++j) {
+        try {
+            plan_op(X, dot, tensor, nb, list[j], cap, plans[j]);
+        } catch (const Error& e) {
+#pragma omp critical
+            { err = e.what(); err_code = e.code; }
+        } catch (const std::exception& e) {
+#pragma omp critical
+            { err = e.what(); err_code = -2; }
         }
-        if (used > cap / 2) flush();
+    }
+    if (err_code) { if (err_code == -3) throw Error(-3, err); throw std::logic_error(err); }
+    int64_t total = 0;
+    for (const OpPlan& pl : plans) total += pl.used;
+    DevVec<double> tmp;
+    tmp.alloc((size_t)std::max<int64_t>(2, std::min(total, cap)));
+    GemmBatch p1, p2;
+    int64_t used = 0;
+    auto flush = [&]() {
+        run_once(p1, eng);
+        run_once(p2, eng);
+        used = 0;
+    };
+    for (OpPlan& pl : plans) {
+        if (used + pl.used > cap) flush();
+        merge(p1, p2, pl, tmp.p + used);
+        used += pl.used;
+        pl = OpPlan();
+        if (used > cap / 2 && total > cap) flush();
     }
     flush();
 }
 
-// ---------------------------------------------------------------------------------------------------------------
-// one blocking step
-// ---------------------------------------------------------------------------------------------------------------
+// symbolic expressions of a list of new operators, generated by the host threads (the generator is read-only)
+enum OpWhat : int { W_H, W_CRE, W_ST, W_A, W_B, W_COPY };
+struct OpSpec { Label label; int what; };
+static std::vector<NewOp> make_ops(const std::vector<OpSpec>& specs, const Gen& gen) {
+    std::vector<NewOp> out(specs.size());
+#pragma omp parallel for schedule(dynamic, 16)
+    for (long j = 0; j < (long)specs.size(); ++j) {
+        const Label& l = specs[j].label;
+        NewOp& o = out[j];
+        o.label = l;
+        switch (specs[j].what) {
+            case W_H: o.expr = gen.H(); break;
+            case W_CRE: o.expr = gen.cre(l.a); break;
+            case W_ST: for (const Term& t : gen.S(l.a)) o.expr.push_back(adjoint(t)); break;
+            case W_A: o.expr = gen.A(l.a, l.b); break;
+            case W_B: o.expr = gen.B(l.a, l.b); break;
+            default: { Term t; t.f.push_back(gen.bf(l)); o.expr.push_back(t); }
+        }
+    }
+    return out;
+}
+
 static bool same_shift(const Label& x, const Label& y) {
     int a, b, c, d;
     op_shift(x, a, b); op_shift(y, c, d);
     return a == c && b == d;
 }
-static Expr single(const Factor& f) { Term t; t.f.push_back(f); return Expr{t}; }
 
 std::unique_ptr<Block> grow(Block& X, const Ham& ham, const MPS& mps, char new_mode, Engine& eng) {
     const bool left = X.side == 'L';
@@ -204,26 +280,22 @@ std::unique_ptr<Block> grow(Block& X, const Ham& ham, const MPS& mps, char new_m
     const std::vector<int> inside = nb.inside(), outside = nb.outside();
     make_temps(ham, X, dot, outside, eng);
     Gen gen(ham, block_info(X), dot);
-    std::vector<NewOp> list;
-    list.push_back({L0(K_H), gen.H()});
-    for (int P : inside) list.push_back({L1(K_C, P), gen.cre(P)});
-    for (int P : outside) {
-        Expr e;
-        for (const Term& t : gen.S(P)) e.push_back(adjoint(t));
-        list.push_back({L1(K_St, P), e});
-    }
+    std::vector<OpSpec> list;
+    list.push_back({L0(K_H), W_H});
+    for (int P : inside) list.push_back({L1(K_C, P), W_CRE});
+    for (int P : outside) list.push_back({L1(K_St, P), W_ST});
     if (X.mode == 'N') {
-        std::vector<NewOp> two;
+        std::vector<OpSpec> two;
         for (size_t a = 0; a < inside.size(); ++a) {
-            for (size_t b = a + 1; b < inside.size(); ++b) two.push_back({L2(K_A, inside[a], inside[b]), gen.A(inside[a], inside[b])});
-            for (int S : inside) two.push_back({L2(K_B, inside[a], S), gen.B(inside[a], S)});
+            for (size_t b = a + 1; b < inside.size(); ++b) two.push_back({L2(K_A, inside[a], inside[b]), W_A});
+            for (int S : inside) two.push_back({L2(K_B, inside[a], S), W_B});
         }
         if (new_mode == 'N') {
             list.insert(list.end(), two.begin(), two.end());
-            rotate_batch(X, dot, tensor, nb, list, false, eng);
+            rotate_batch(X, dot, tensor, nb, make_ops(list, gen), false, eng);
         } else {                                               // grow the normal operators, then convert
-            rotate_batch(X, dot, tensor, nb, list, false, eng);
-            rotate_batch(X, dot, tensor, nb, two, true, eng);
+            rotate_batch(X, dot, tensor, nb, make_ops(list, gen), false, eng);
+            rotate_batch(X, dot, tensor, nb, make_ops(two, gen), true, eng);
             std::vector<LinSpec> specs;
             for (size_t a = 0; a < outside.size(); ++a) {
                 for (size_t b = a + 1; b < outside.size(); ++b) {
@@ -255,36 +327,36 @@ std::unique_ptr<Block> grow(Block& X, const Ham& ham, const MPS& mps, char new_m
         if (new_mode != 'C') throw std::logic_error("grow: complementary -> normal is not supported");
         std::vector<char> in_x(2 * X.k, 0);
         for (int P : X.inside()) in_x[P] = 1;
-        std::vector<NewOp> mixed;                              // new normal operators with one index on the new site
+        std::vector<OpSpec> mixed;                             // new normal operators with one index on the new site
         for (size_t a = 0; a < inside.size(); ++a) {
             for (size_t b = a + 1; b < inside.size(); ++b)
-                if (!(in_x[inside[a]] && in_x[inside[b]])) mixed.push_back({L2(K_A, inside[a], inside[b]), gen.A(inside[a], inside[b])});
+                if (!(in_x[inside[a]] && in_x[inside[b]])) mixed.push_back({L2(K_A, inside[a], inside[b]), W_A});
             for (int S : inside)
-                if (!(in_x[inside[a]] && in_x[S])) mixed.push_back({L2(K_B, inside[a], S), gen.B(inside[a], S)});
+                if (!(in_x[inside[a]] && in_x[S])) mixed.push_back({L2(K_B, inside[a], S), W_B});
         }
         std::vector<LinSpec> specs;
         for (size_t a = 0; a < outside.size(); ++a) {
             for (size_t b = a + 1; b < outside.size(); ++b) {
                 const Label l = L2(K_Pt, outside[a], outside[b]);
-                list.push_back({l, single(gen.bf(l))});
+                list.push_back({l, W_COPY});
                 LinSpec s; s.dst = l;
-                for (const NewOp& m : mixed)
+                for (const OpSpec& m : mixed)
                     if (m.label.kind == K_A && same_shift(m.label, l))
                         s.items.push_back({-ham.w(outside[a], outside[b], m.label.a, m.label.b), m.label});
                 specs.push_back(s);
             }
             for (int S : outside) {
                 const Label l = L2(K_Q, outside[a], S);
-                list.push_back({l, single(gen.bf(l))});
+                list.push_back({l, W_COPY});
                 LinSpec s; s.dst = l;
-                for (const NewOp& m : mixed)
+                for (const OpSpec& m : mixed)
                     if (m.label.kind == K_B && same_shift(m.label, l))
                         s.items.push_back({ham.w(outside[a], m.label.a, m.label.b, S), m.label});
                 specs.push_back(s);
             }
         }
-        rotate_batch(X, dot, tensor, nb, list, false, eng);
-        rotate_batch(X, dot, tensor, nb, mixed, true, eng);
+        rotate_batch(X, dot, tensor, nb, make_ops(list, gen), false, eng);
+        rotate_batch(X, dot, tensor, nb, make_ops(mixed, gen), true, eng);
         lincomb(nb, specs, true, eng);
         nb.drop_temps();
     }
@@ -301,16 +373,16 @@ std::unique_ptr<Block> grow_normal(Block& X, const Ham& ham, const Basis& new_ba
     Gen gen(ham, block_info(X), dot);
     const std::vector<int> inside = nbp->inside();
     auto paired = [&](int P) { const int s = P >> 1; return s >= pair_lo && s < pair_hi; };
-    std::vector<NewOp> list;
+    std::vector<OpSpec> list;
     for (size_t a = 0; a < inside.size(); ++a) {
-        list.push_back({L1(K_C, inside[a]), gen.cre(inside[a])});
+        list.push_back({L1(K_C, inside[a]), W_CRE});
         if (!paired(inside[a])) continue;
         for (size_t b = a + 1; b < inside.size(); ++b)
-            if (paired(inside[b])) list.push_back({L2(K_A, inside[a], inside[b]), gen.A(inside[a], inside[b])});
+            if (paired(inside[b])) list.push_back({L2(K_A, inside[a], inside[b]), W_A});
         for (int S : inside)
-            if (paired(S)) list.push_back({L2(K_B, inside[a], S), gen.B(inside[a], S)});
+            if (paired(S)) list.push_back({L2(K_B, inside[a], S), W_B});
     }
-    rotate_batch(X, dot, tensor, *nbp, list, false, eng);
+    rotate_batch(X, dot, tensor, *nbp, make_ops(list, gen), false, eng);
     return nbp;
 }
 

@@ -46,7 +46,10 @@ void launch_seg_gemm_tma(const Task* tasks, const Seg* segs, const Tile* tiles, 
 
 // ---- vector kernels (Davidson; HBM-bound) ---------------------------------------------------------------------------
 // out[j] = sum_i x[i] * Y[j*ldy + i], j < m  (deterministic two-stage reduction; out is a device array of m doubles)
-void launch_multi_dot(const double* x, const double* Y, int64_t ldy, int m, int64_t n, double* out, cudaStream_t st);
+// scratch: multi_dot_scratch() doubles owned by the caller (one per context: no process-global buffers)
+int64_t multi_dot_scratch();
+void launch_multi_dot(const double* x, const double* Y, int64_t ldy, int m, int64_t n, double* out, double* scratch,
+                      cudaStream_t st);
 constexpr int COMBINE_MAX = 32;
 // out[i] = beta * out[i] + sum_{j<m} coef_host[j] * V[j*ldv + i],  m <= COMBINE_MAX
 void launch_combine(double* out, double beta, const double* V, int64_t ldv, int m, const double* coef_host, int64_t n,

@@ -657,7 +657,7 @@ void rdm12(Engine& eng, double* gamma, double* Gamma) {
     clone_site(mps.sites[0], mps.bonds[0], mps.bonds[1], centre, eng);
     DevVec<double> scal;
     scal.alloc(1);
-    launch_multi_dot(centre.data.p, centre.data.p, centre.nnz, 1, centre.nnz, scal.p, eng.stream);
+    launch_multi_dot(centre.data.p, centre.data.p, centre.nnz, 1, centre.nnz, scal.p, eng.red_scratch.p, eng.stream);
     eng.launches += 2;
     double nrm2 = 0.0;
     cuda_check(cudaMemcpyAsync(&nrm2, scal.p, 8, cudaMemcpyDeviceToHost, eng.stream), "norm");

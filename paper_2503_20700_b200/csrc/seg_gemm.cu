@@ -241,12 +241,8 @@ __global__ void __launch_bounds__(NT) seg_gemm_kernel(const Task* __restrict__ t
 
 void launch_seg_gemm(const Task* d_tasks, const Seg* d_segs, const Tile* d_tiles, int ntiles, cudaStream_t stream) {
     if (ntiles <= 0) return;
-    static bool configured = false;
     const int smem_bytes = ST * STAGE_DOUBLES * (int)sizeof(double);
-    if (!configured) {
-        cudaFuncSetAttribute(seg_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
-        configured = true;
-    }
+    cudaFuncSetAttribute(seg_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);   // per device: not cached (test / fallback kernel)
     seg_gemm_kernel<<<ntiles, NT, smem_bytes, stream>>>(d_tasks, d_segs, d_tiles, ntiles);
 }
 

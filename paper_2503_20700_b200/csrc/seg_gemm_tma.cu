@@ -16,6 +16,8 @@
 
 #include <cuda_runtime.h>
 
+#include <atomic>
+
 #include <cstdint>
 
 namespace dmrg {
@@ -408,18 +410,21 @@ seg_gemm_tma_kernel(const Task* __restrict__ tasks, const Seg* __restrict__ segs
 void launch_seg_gemm_tma(const Task* d_tasks, const Seg* d_segs, const Tile* d_tiles, int ntiles, int* d_counter,
                          cudaStream_t stream) {
     if (ntiles <= 0) return;
-    static bool configured = false;
-    static int grid_cap = 148 * 3;
+    // launch configuration cached per device (several contexts on several devices may live in one process)
+    constexpr int MAX_DEV = 64;
+    static std::atomic<int> grid_caps[MAX_DEV];
     const int smem_bytes = ST2 * STAGE_DOUBLES * (int)sizeof(double);
-    if (!configured) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    int grid_cap = (dev >= 0 && dev < MAX_DEV) ? grid_caps[dev].load(std::memory_order_acquire) : 0;
+    if (grid_cap == 0) {
         cudaFuncSetAttribute(seg_gemm_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
-        int dev = 0, sms = 148, per_sm = 3;
-        cudaGetDevice(&dev);
+        int sms = 148, per_sm = 3;
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, seg_gemm_tma_kernel, NT2, smem_bytes);
         if (per_sm < 1) per_sm = 1;
         grid_cap = sms * per_sm;                            // persistent: one CTA per resident slot
-        configured = true;
+        if (dev >= 0 && dev < MAX_DEV) grid_caps[dev].store(grid_cap, std::memory_order_release);
     }
     cudaMemsetAsync(d_counter, 0, sizeof(int), stream);
     const int grid = ntiles < grid_cap ? ntiles : grid_cap;

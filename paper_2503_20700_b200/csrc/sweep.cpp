@@ -7,6 +7,8 @@
 #include <cstdlib>
 #include <cmath>
 
+#include <omp.h>
+
 #include "core.hpp"
 
 namespace dmrg {
@@ -59,7 +61,7 @@ DavidsonResult davidson(HeffPlan& p, double* x_dev, Engine& eng) {
     scal.alloc(COMBINE_MAX + 2);
     std::vector<double> hs((size_t)COMBINE_MAX + 2);
     auto dots = [&](const double* x, const double* Y, int m) {          // -> hs[0..m)
-        launch_multi_dot(x, Y, n, m, n, scal.p, st);
+        launch_multi_dot(x, Y, n, m, n, scal.p, eng.red_scratch.p, st);
         eng.launches += 2;
         cuda_check(cudaMemcpyAsync(hs.data(), scal.p, sizeof(double) * m, cudaMemcpyDeviceToHost, st), "dots");
         cuda_check(cudaStreamSynchronize(st), "dots");
@@ -210,7 +212,7 @@ void split_theta(MPS& mps, int i, const HeffPlan& p, const double* theta, int D,
     // norm of theta (the kept state is rescaled to unit norm afterwards)
     DevVec<double> scal;
     scal.alloc(1);
-    launch_multi_dot(theta, theta, p.nnz, 1, p.nnz, scal.p, st); eng.launches += 2;
+    launch_multi_dot(theta, theta, p.nnz, 1, p.nnz, scal.p, eng.red_scratch.p, st); eng.launches += 2;
     double nrm2 = 0.0;
     cuda_check(cudaMemcpyAsync(&nrm2, scal.p, 8, cudaMemcpyDeviceToHost, st), "norm");
     cuda_check(cudaStreamSynchronize(st), "norm");
@@ -225,25 +227,52 @@ void split_theta(MPS& mps, int i, const HeffPlan& p, const double* theta, int D,
         for (auto& rc : sc.rows) { sc.roff.push_back(sc.nr); sc.nr += bl[rc.first].d; }
         for (auto& cc : sc.cols) { sc.coff.push_back(sc.nc); sc.nc += br[cc.second].d; }
         sc.rk = std::min(sc.nr, sc.nc);
-        sc.M.alloc((size_t)sc.nr * sc.nc);
-        cuda_check(cudaMemsetAsync(sc.M.p, 0, (size_t)sc.nr * sc.nc * 8, st), "memset");
-        for (size_t ri = 0; ri < sc.rows.size(); ++ri)
-            for (size_t ci = 0; ci < sc.cols.size(); ++ci) {
-                const int idx = p.lookup[sc.rows[ri].first * 16 + sc.rows[ri].second * 4 + sc.cols[ci].first];
-                if (idx < 0 || p.layout[idx].r != sc.cols[ci].second) continue;
-                const PsiBlock& b = p.layout[idx];
-                launch_copy2d(sc.M.p + (size_t)sc.roff[ri] * sc.nc + sc.coff[ci], sc.nc, theta + b.off, b.cols, b.rows,
-                              b.cols, inv_nrm, nullptr, nullptr, st);
-                eng.launches++;
-            }
-        sc.U.alloc((size_t)sc.nr * sc.rk); sc.S.alloc((size_t)sc.rk); sc.Vt.alloc((size_t)sc.rk * sc.nc);
-        svd_rowmajor(eng.svd, sc.M.p, sc.nr, sc.nc, sc.U.p, sc.S.p, sc.Vt.p, st);
-        sc.sv.resize(sc.rk);
-        cuda_check(cudaMemcpyAsync(sc.sv.data(), sc.S.p, (size_t)sc.rk * 8, cudaMemcpyDeviceToHost, st), "sv");
-        cuda_check(cudaStreamSynchronize(st), "sv");
-        for (int j = 0; j < sc.rk; ++j) pool.push_back({sc.sv[j], (int)order.size(), j});
         order.push_back(&sc);
     }
+    // The sector SVDs are independent and individually too small to fill the device: a few host threads run them
+    // concurrently, each on its own stream and cuSOLVER handle (theta is complete: Davidson ended synchronised).
+    // Largest sectors first.
+    const int nthreads = 4;
+    eng.ensure_svd_pool(nthreads);
+    std::vector<int> by_size(order.size());
+    for (size_t j = 0; j < order.size(); ++j) by_size[j] = (int)j;
+    std::stable_sort(by_size.begin(), by_size.end(), [&](int x, int y) {
+        return (double)order[x]->nr * order[x]->nc * order[x]->rk > (double)order[y]->nr * order[y]->nc * order[y]->rk; });
+    std::string err;
+    int64_t nlaunch = 0;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads) reduction(+ : nlaunch)
+    for (long jj = 0; jj < (long)by_size.size(); ++jj) {
+        try {
+            const int tid = omp_get_thread_num();
+            cudaStream_t ts = eng.svd_streams[tid];
+            cuda_check(cudaSetDevice(eng.opt.device_id), "cudaSetDevice");
+            Sec& sc = *order[by_size[jj]];
+            sc.M.alloc((size_t)sc.nr * sc.nc);
+            cuda_check(cudaMemsetAsync(sc.M.p, 0, (size_t)sc.nr * sc.nc * 8, ts), "memset");
+            for (size_t ri = 0; ri < sc.rows.size(); ++ri)
+                for (size_t ci = 0; ci < sc.cols.size(); ++ci) {
+                    const int ix = p.lookup[sc.rows[ri].first * 16 + sc.rows[ri].second * 4 + sc.cols[ci].first];
+                    if (ix < 0 || p.layout[ix].r != sc.cols[ci].second) continue;
+                    const PsiBlock& b = p.layout[ix];
+                    launch_copy2d(sc.M.p + (size_t)sc.roff[ri] * sc.nc + sc.coff[ci], sc.nc, theta + b.off, b.cols, b.rows,
+                                  b.cols, inv_nrm, nullptr, nullptr, ts);
+                    nlaunch++;
+                }
+            sc.U.alloc((size_t)sc.nr * sc.rk); sc.S.alloc((size_t)sc.rk); sc.Vt.alloc((size_t)sc.rk * sc.nc);
+            svd_rowmajor(eng.svd_pool[tid], sc.M.p, sc.nr, sc.nc, sc.U.p, sc.S.p, sc.Vt.p, ts);
+            sc.sv.resize(sc.rk);
+            cuda_check(cudaMemcpyAsync(sc.sv.data(), sc.S.p, (size_t)sc.rk * 8, cudaMemcpyDeviceToHost, ts), "sv");
+            cuda_check(cudaStreamSynchronize(ts), "sv");
+            sc.M.release();
+        } catch (const std::exception& e) {
+#pragma omp critical
+            err = e.what();
+        }
+    }
+    if (!err.empty()) throw Error(-4, "split: " + err);
+    eng.launches += nlaunch;
+    for (size_t j = 0; j < order.size(); ++j)
+        for (int q = 0; q < order[j]->rk; ++q) pool.push_back({order[j]->sv[q], (int)j, q});
     std::vector<int> idx(pool.size());
     for (size_t t = 0; t < idx.size(); ++t) idx[t] = (int)t;
     std::stable_sort(idx.begin(), idx.end(), [&](int x, int y) { return pool[x].sv > pool[y].sv; });
@@ -320,6 +349,15 @@ void split_theta(MPS& mps, int i, const HeffPlan& p, const double* theta, int D,
 // per block and pass - renormalisation is a few percent of a sweep).  Checkpoints may additionally be spilled to
 // pinned host memory with an asynchronous copy on a separate stream and fetched back when their segment is entered.
 // ---------------------------------------------------------------------------------------------------------------
+void Engine::ensure_svd_pool(int n) {
+    while ((int)svd_pool.size() < n) {
+        cudaStream_t ts = nullptr;
+        cuda_check(cudaStreamCreateWithFlags(&ts, cudaStreamNonBlocking), "cudaStreamCreate");
+        svd_streams.push_back(ts);
+        svd_pool.push_back(svd_create(ts, opt.svd_qr == 0));
+    }
+}
+
 static double wall() { return std::chrono::duration<double>(std::chrono::steady_clock::now().time_since_epoch()).count(); }
 
 static int64_t g_device_bytes_env(const Engine& eng) {         // device bytes held by environment blocks right now

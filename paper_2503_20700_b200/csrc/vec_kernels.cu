@@ -219,13 +219,12 @@ int grid_for(int64_t n, int threads) {
     return (int)b;
 }
 
-double* g_partial = nullptr;    // scratch of the two-stage reductions (COMBINE_MAX x RED_BLOCKS doubles)
-
 }  // namespace
 
-void launch_multi_dot(const double* x, const double* Y, int64_t ldy, int m, int64_t n, double* out, cudaStream_t st) {
+int64_t multi_dot_scratch() { return (int64_t)64 * RED_BLOCKS; }
+void launch_multi_dot(const double* x, const double* Y, int64_t ldy, int m, int64_t n, double* out, double* g_partial,
+                      cudaStream_t st) {
     if (m <= 0) return;
-    if (!g_partial) cudaMalloc(&g_partial, sizeof(double) * 64 * RED_BLOCKS);
     int nb = grid_for(n, RED_THREADS);
     if (nb > RED_BLOCKS) nb = RED_BLOCKS;
     for (int j0 = 0; j0 < m; j0 += 64) {
@@ -289,11 +288,8 @@ void launch_stack_dots(const double* S, int64_t lds, int nrows, const double* M,
     const int grid = (int)(items < 148 * 2 * 4 ? items : 148 * 2 * 4);
     const int NCt = nc <= 1 ? 1 : (nc <= 2 ? 2 : (nc <= 4 ? 4 : 8));
     const int smem = NCt * SD_KC * (int)sizeof(double);
-    static bool configured = false;
-    if (!configured) {
-        cudaFuncSetAttribute(stack_dots_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 8 * SD_KC * 8);
-        configured = true;
-    }
+    // the attribute is per device: set it on every launch (a cheap host-side call) instead of caching a process-wide flag
+    if (NCt == 8) cudaFuncSetAttribute(stack_dots_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 8 * SD_KC * 8);
     if (K <= 0) { cudaMemsetAsync(scratch, 0, sizeof(double) * (size_t)nspans * nrows * nc, st); }
     else if (NCt == 1) stack_dots_kernel<1><<<grid, SD_WARPS * 32, smem, st>>>(S, lds, nrows, M, ldm, nc, K, span, nspans, scratch);
     else if (NCt == 2) stack_dots_kernel<2><<<grid, SD_WARPS * 32, smem, st>>>(S, lds, nrows, M, ldm, nc, K, span, nspans, scratch);
