@@ -267,15 +267,18 @@ def time_sweep_rdm(P, torch, peaks, cid, D, nsweep, rdm=True, **opts):
         except P.binding.DmrgError as ex:                 # e.g. the environment stack does not fit the device
             rec["sweep"] = {"error": str(ex), "s_per_sweep": secs}
             return rec
-        mv = int(sum(b["n_matvec"] for b in r["bonds"]))
-        fl = float(sum(b["n_matvec"] * b["f_alg"] for b in r["bonds"]))
-        tmv = float(sum(b["seconds_matvec"] for b in r["bonds"]))
-        rec["sweep"] = {"s_per_sweep": secs, "energy_last_eh": e + cfg["e_core"], "matvecs_last_sweep": mv,
+        if r is None:
+            rec["sweep"] = {"skipped": "--sweeps 0: the RDM pass runs on the seeded random MPS"}
+        else:
+          mv = int(sum(b["n_matvec"] for b in r["bonds"]))
+          fl = float(sum(b["n_matvec"] * b["f_alg"] for b in r["bonds"]))
+          tmv = float(sum(b["seconds_matvec"] for b in r["bonds"]))
+          rec["sweep"] = {"s_per_sweep": secs, "energy_last_eh": e + cfg["e_core"], "matvecs_last_sweep": mv,
                         "matvec_seconds_last_sweep": tmv, "matvec_f_alg_last_sweep": fl,
                         "matvec_tflops_last_sweep": fl / tmv / 1e12 if tmv > 0 else None,
                         "max_kept": int(max(b["kept"] for b in r["bonds"])),
-                        "unconverged_bonds": int(sum(1 - b["converged"] for b in r["bonds"])),
-                        "phases_last_sweep": phases[-1]}
+                          "unconverged_bonds": int(sum(1 - b["converged"] for b in r["bonds"])),
+                          "phases_last_sweep": phases[-1]}
         if not rdm:
             return rec
         try:

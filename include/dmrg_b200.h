@@ -45,7 +45,7 @@ typedef struct dmrg_options {
      * checkpoints are moved to pinned host memory by asynchronous copies and fetched back when needed.  Results do not
      * depend on these settings (the recomputed blocks are bit-identical). */
     int64_t hbm_budget_bytes;     /* default 0 = automatic (55 % of the free device memory): bytes the stack may hold */
-    int64_t host_budget_bytes;    /* default 0 = automatic (96 GiB): pinned host bytes for spilled checkpoints        */
+    int64_t host_budget_bytes;    /* default 0 = automatic (64 GiB): pinned host bytes for spilled checkpoints        */
     int32_t host_spill;           /* default 0; 1: checkpoints may be spilled to pinned host memory                    */
     int32_t env_stride;           /* default 0 = automatic from the budgets; 1 = keep every block; s: every s-th       */
     /* Dynamic block state selection: dbss_eps > 0 keeps, at every bond, the fewest states
@@ -56,7 +56,7 @@ typedef struct dmrg_options {
     int32_t svd_qr;               /* default 0: one-sided Jacobi SVD (cuSOLVER gesvdj, gesvd fallback); 1: gesvd       */
     int32_t host_maps;            /* default 0: block maps built on the device; 1: host reference builder (A/B tests)  */
     int32_t generic_gemm;         /* default 0; 1: always the cp.async GEMM kernel instead of the bulk-copy one (A/B)  */
-    int32_t reserved0;
+    int32_t eigensolver;          /* default 0: Davidson; 1: Lanczos (PAPER.md:179 names both); same tolerance fields  */
 } dmrg_options;
 
 /* Neutral MPS exchange format (host memory, caller-owned, flat arrays).
@@ -148,6 +148,14 @@ int dmrg_heff_stats(dmrg_ctx* ctx, int i, double* f_alg, double* f_exec, double*
  * MPS, which must be right-canonical before the first sweep.  records: caller array of 2(k-1) entries (nullable).
  * Returns DMRG_ENOCONV (warning) if any Davidson hit max_iter. */
 int dmrg_sweep(dmrg_ctx* ctx, int D, dmrg_sweep_result* result, dmrg_bond_record* records);
+
+/* Sweeps at bond dimension D until the stopping rule of PAPER.md:179 holds - the sweep energies (energy_last) of three
+ * subsequent sweeps differ by less than eps_sweep, |E_s - E_{s-1}| < eps and |E_{s-1} - E_{s-2}| < eps (reading S34) - or
+ * max_sweeps sweeps have run.  *n_sweeps (HOST) receives the number of sweeps, energies (HOST, max_sweeps doubles,
+ * nullable) their energy_last; last / last_records as in dmrg_sweep for the final sweep.  Returns DMRG_ENOCONV if the
+ * rule was not met within max_sweeps (or a Davidson hit max_iter in the final sweep). */
+int dmrg_solve(dmrg_ctx* ctx, int D, double eps_sweep, int max_sweeps, int32_t* n_sweeps, double* energies,
+               dmrg_sweep_result* last, dmrg_bond_record* last_records);
 
 /* Phase timers and environment-stack accounting of the last dmrg_sweep call (seconds per phase).
  * seconds_environments = restore + regrow + the initial right stack; seconds_spill_wait = time the host waited for an

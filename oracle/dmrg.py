@@ -710,6 +710,55 @@ def davidson(apply, diag, x0, tol=1e-7, max_iter=100, max_subspace=20):
     return theta, u / np.linalg.norm(u), nmv, rn, False
 
 
+def lanczos(apply, x0, tol=1e-7, max_iter=100, max_subspace=20):
+    """Lowest eigenpair of the symmetric operator `apply` by the Lanczos method, the paper's other local eigensolver
+    ("Lanczos and Davidson diagonalization methods"; reading S33): Krylov vectors
+    v_{j+1} beta_{j+1} = H v_j - alpha_j v_j - beta_j v_{j-1}, re-orthogonalised against all stored vectors (twice),
+    Rayleigh-Ritz on the tridiagonal matrix, residual norm beta_{j+1} |s_j|, restart from the Ritz vector when
+    max_subspace vectors are stored.  Returns (theta, u, n_matvec, residual_norm, ok) like davidson()."""
+    v = x0 / np.linalg.norm(x0)
+    V, alphas, betas = [v], [], []
+    nmv = 0
+    theta, u, rn = 0.0, v, np.inf
+    for _ in range(max_iter):
+        w = apply(V[-1])
+        nmv += 1
+        alphas.append(float(V[-1] @ w))
+        w = w - alphas[-1] * V[-1]
+        if len(V) > 1:
+            w = w - betas[-1] * V[-2]
+        for _gs in range(2):
+            for vv in V:
+                w = w - (vv @ w) * vv
+        beta = float(np.linalg.norm(w))
+        m = len(V)
+        T = np.diag(alphas) + np.diag(betas, 1) + np.diag(betas, -1)
+        ev, es = np.linalg.eigh(T)
+        theta, s = ev[0], es[:, 0]
+        u = s @ np.array(V)
+        rn = abs(beta * s[-1])
+        if rn <= tol:
+            return theta, u / np.linalg.norm(u), nmv, rn, True
+        if beta < 1e-14:
+            break
+        if m >= max_subspace:
+            V, alphas, betas = [u / np.linalg.norm(u)], [], []
+            continue
+        betas.append(beta)
+        V.append(w / beta)
+    return theta, u / np.linalg.norm(u), nmv, rn, False
+
+
+def sweeps_converged(energies, eps_sweep):
+    """Stopping rule of the sweep loop ("terminated when the energy difference between three subsequent
+    sweeps falls below ... eps_sweep"; reading S34): true once the last three sweep energies E_{s-2}, E_{s-1}, E_s
+    differ pairwise-consecutively by less than eps_sweep."""
+    if len(energies) < 3:
+        return False
+    a, b, c = energies[-3:]
+    return abs(b - a) < eps_sweep and abs(c - b) < eps_sweep
+
+
 # ----------------------------------------------------------------------------------------------------------------
 # decomposition and truncation (reading S14) and the two-site sweep (readings S12, S16-S18)
 # ----------------------------------------------------------------------------------------------------------------
@@ -830,7 +879,7 @@ class SweepEngine:
     over bonds 0..k-2 then backward pass k-2..0 (reading S12)."""
 
     def __init__(self, h, eri, mps, davidson_tol=1e-7, davidson_max_iter=100, davidson_max_subspace=20, dbss_eps=0.0,
-                 dbss_dmin=0):
+                 dbss_dmin=0, eigensolver="davidson"):
         self.ham = Ham(h, eri)
         self.k = self.ham.k
         self.mps = dict(mps)
@@ -839,6 +888,7 @@ class SweepEngine:
         self.mps["gauge"] = list(mps["gauge"])
         self.opts = dict(tol=davidson_tol, max_iter=davidson_max_iter, max_subspace=davidson_max_subspace)
         self.dbss = dict(dbss_eps=dbss_eps, dbss_dmin=dbss_dmin)
+        self.eigensolver = eigensolver
         self.L = {0: empty_block("L", self.k, self.mps)}
         self.R = build_right(self.mps, self.ham, 2)
         self.log = []
@@ -847,7 +897,10 @@ class SweepEngine:
         mps, ham = self.mps, self.ham
         H = Heff(self.L[i], self.R[i + 2], ham, i)
         guess = blocks_to_flat(H.layout, H.nnz, two_site_tensor(mps, i))
-        theta, u, nmv, rn, ok = davidson(H.apply, H.diagonal(), guess, **self.opts)
+        if self.eigensolver == "lanczos":
+            theta, u, nmv, rn, ok = lanczos(H.apply, guess, **self.opts)
+        else:
+            theta, u, nmv, rn, ok = davidson(H.apply, H.diagonal(), guess, **self.opts)
         ub = flat_to_blocks(H.layout, u)
         mid, Ab, Bb, trunc, kept = split_theta(ub, mps["bonds"][i], mps["bonds"][i + 2], D, direction, **self.dbss)
         mps["bonds"][i + 1] = mid
@@ -870,6 +923,15 @@ class SweepEngine:
         for i in range(self.k - 2, -1, -1):
             recs.append(self._optimise(i, D, "bwd"))
         return dict(energy_last=recs[-1]["energy"], energy_min=min(r["energy"] for r in recs), bonds=recs)
+
+    def solve(self, D, eps_sweep, max_sweeps):
+        """Sweeps until sweeps_converged (reading S34) or max_sweeps; returns the list of sweep results."""
+        out = []
+        while len(out) < max_sweeps:
+            out.append(self.sweep(D))
+            if sweeps_converged([r["energy_last"] for r in out], eps_sweep):
+                break
+        return out
 
 
 # ----------------------------------------------------------------------------------------------------------------

@@ -28,7 +28,7 @@ class dmrg_options(C.Structure):
                 ("keep_env_stack", C.c_int32), ("workspace_bytes", C.c_int64),
                 ("hbm_budget_bytes", C.c_int64), ("host_budget_bytes", C.c_int64), ("host_spill", C.c_int32),
                 ("env_stride", C.c_int32), ("dbss_eps", C.c_double), ("dbss_dmin", C.c_int32), ("split_k", C.c_int32),
-                ("svd_qr", C.c_int32), ("host_maps", C.c_int32), ("generic_gemm", C.c_int32), ("reserved0", C.c_int32)]
+                ("svd_qr", C.c_int32), ("host_maps", C.c_int32), ("generic_gemm", C.c_int32), ("eigensolver", C.c_int32)]
 
 
 class dmrg_mps_blob(C.Structure):
@@ -58,7 +58,7 @@ class dmrg_sweep_result(C.Structure):
 
 EXPORTS = ["dmrg_default_options", "dmrg_create", "dmrg_destroy", "dmrg_last_error", "dmrg_mps_import",
            "dmrg_mps_export", "dmrg_prepare_bond", "dmrg_heff_layout", "dmrg_heff_apply", "dmrg_heff_diag",
-           "dmrg_heff_stats", "dmrg_sweep", "dmrg_sweep_stats", "dmrg_rdm12", "dmrg_rdm_stats", "dmrg_launch_count", "dmrg_flops_total", "dmrg_device_bytes",
+           "dmrg_heff_stats", "dmrg_sweep", "dmrg_solve", "dmrg_sweep_stats", "dmrg_rdm12", "dmrg_rdm_stats", "dmrg_launch_count", "dmrg_flops_total", "dmrg_device_bytes",
            "dmrg_grouped_gemm", "dmrg_stack_dots"]
 
 lib.dmrg_last_error.restype = C.c_char_p
@@ -193,6 +193,20 @@ def dmrg_sweep(ctx, D, k):
     bonds = [dict((f, getattr(r, f)) for f, _ in dmrg_bond_record._fields_) for r in recs[:res.n_records]]
     return dict(energy_last=res.energy_last, energy_min=res.energy_min, seconds=res.seconds,
                 warnings=res.warnings, status=rc, bonds=bonds)
+
+
+def dmrg_solve(ctx, D, k, eps_sweep, max_sweeps):
+    """Sweeps until three subsequent sweep energies differ by less than eps_sweep or max_sweeps ->
+    dict(n_sweeps, energies, converged, last = result dict of the final sweep as returned by dmrg_sweep)."""
+    res = dmrg_sweep_result()
+    recs = (dmrg_bond_record * (2 * (k - 1)))()
+    n = C.c_int32(0)
+    en = np.zeros(max_sweeps)
+    rc = _check(ctx, lib.dmrg_solve(ctx, int(D), C.c_double(eps_sweep), int(max_sweeps), C.byref(n), _ptr(en), C.byref(res), recs))
+    bonds = [dict((f, getattr(r, f)) for f, _ in dmrg_bond_record._fields_) for r in recs[:res.n_records]]
+    return dict(n_sweeps=n.value, energies=en[:n.value].copy(), status=rc,
+                last=dict(energy_last=res.energy_last, energy_min=res.energy_min, seconds=res.seconds,
+                          warnings=res.warnings, bonds=bonds))
 
 
 class dmrg_sweep_stats_t(C.Structure):

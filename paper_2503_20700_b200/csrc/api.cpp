@@ -77,7 +77,7 @@ void dmrg_default_options(dmrg_options* o) {
     o->workspace_bytes = 0;
     o->hbm_budget_bytes = 0; o->host_budget_bytes = 0; o->host_spill = 0; o->env_stride = 0;
     o->dbss_eps = 0.0; o->dbss_dmin = 0; o->split_k = 0; o->svd_qr = 0; o->host_maps = 0; o->generic_gemm = 0;
-    o->reserved0 = 0;
+    o->eigensolver = 0;
 }
 
 int dmrg_create(dmrg_ctx** out, int k, int n_elec, int two_sz, const double* h, const double* eri,
@@ -109,11 +109,13 @@ int dmrg_create(dmrg_ctx** out, int k, int n_elec, int two_sz, const double* h, 
             eng.opt.dbss_eps = opt->dbss_eps; eng.opt.dbss_dmin = opt->dbss_dmin;
             eng.opt.split_k = opt->split_k; eng.opt.svd_qr = opt->svd_qr;
             eng.host_maps = opt->host_maps != 0; eng.force_generic_gemm = opt->generic_gemm != 0;
+            eng.opt.eigensolver = opt->eigensolver;
         }
         if (eng.opt.davidson_max_subspace < 2 || eng.opt.davidson_max_subspace > COMBINE_MAX ||
             eng.opt.davidson_max_iter < 1 || !(eng.opt.davidson_tol > 0) || eng.opt.env_stride < 0 ||
             eng.opt.split_k < 0 || eng.opt.split_k > 16 || eng.opt.dbss_eps < 0 || eng.opt.dbss_dmin < 0 ||
-            eng.opt.hbm_budget_bytes < 0 || eng.opt.host_budget_bytes < 0) { delete ctx; return DMRG_EINVAL; }
+            eng.opt.hbm_budget_bytes < 0 || eng.opt.host_budget_bytes < 0 || eng.opt.eigensolver < 0 ||
+            eng.opt.eigensolver > 1) { delete ctx; return DMRG_EINVAL; }
         int ndev = 0;
         if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= eng.opt.device_id) { delete ctx; return DMRG_ECUDA; }
         cuda_check(cudaSetDevice(eng.opt.device_id), "cudaSetDevice");
@@ -351,8 +353,7 @@ int dmrg_heff_stats(dmrg_ctx* ctx, int i, double* f_alg, double* f_exec, double*
     API_END
 }
 
-int dmrg_sweep(dmrg_ctx* ctx, int D, dmrg_sweep_result* result, dmrg_bond_record* records) {
-    API_BEGIN(ctx)
+static int run_sweep(Engine& eng, int D, dmrg_sweep_result* result, dmrg_bond_record* records) {
     if (!eng.have_mps) return fail(eng, DMRG_ESTATE, "sweep: import an MPS first");
     if (D < 1) return fail(eng, DMRG_EINVAL, "sweep: D < 1");
     if (eng.k < 2) return fail(eng, DMRG_EINVAL, "sweep: needs at least two sites");
@@ -385,6 +386,34 @@ int dmrg_sweep(dmrg_ctx* ctx, int D, dmrg_sweep_result* result, dmrg_bond_record
             o.f_alg = r.f_alg; o.seconds = r.seconds; o.seconds_matvec = r.seconds_matvec;
         }
     return warnings ? DMRG_ENOCONV : DMRG_OK;
+}
+
+int dmrg_sweep(dmrg_ctx* ctx, int D, dmrg_sweep_result* result, dmrg_bond_record* records) {
+    API_BEGIN(ctx)
+    return run_sweep(eng, D, result, records);
+    API_END
+}
+
+int dmrg_solve(dmrg_ctx* ctx, int D, double eps_sweep, int max_sweeps, int32_t* n_sweeps, double* energies,
+               dmrg_sweep_result* last, dmrg_bond_record* last_records) {
+    API_BEGIN(ctx)
+    if (!(eps_sweep > 0.0) || max_sweeps < 1 || !n_sweeps) return fail(eng, DMRG_EINVAL, "solve: bad eps_sweep / max_sweeps / n_sweeps");
+    *n_sweeps = 0;
+    std::vector<double> e;
+    dmrg_sweep_result res;
+    int rc = DMRG_OK;
+    bool met = false;
+    while ((int)e.size() < max_sweeps) {
+        rc = run_sweep(eng, D, &res, last_records);
+        if (rc < 0) return rc;
+        e.push_back(res.energy_last);
+        if (energies) energies[e.size() - 1] = res.energy_last;
+        *n_sweeps = (int32_t)e.size();
+        const size_t s = e.size();
+        if (s >= 3 && std::fabs(e[s - 2] - e[s - 3]) < eps_sweep && std::fabs(e[s - 1] - e[s - 2]) < eps_sweep) { met = true; break; }
+    }
+    if (last) *last = res;
+    return (!met || rc == DMRG_ENOCONV) ? DMRG_ENOCONV : DMRG_OK;
     API_END
 }
 

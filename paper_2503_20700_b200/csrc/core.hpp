@@ -222,13 +222,14 @@ struct Options {
     int device_id = 0;
     int64_t workspace_bytes = 0;
     int64_t hbm_budget_bytes = 0;                 // device bytes the environment stack of a sweep may hold (0 = automatic)
-    int64_t host_budget_bytes = 0;                // pinned host bytes for spilled checkpoints (0 = automatic: 96 GiB)
+    int64_t host_budget_bytes = 0;                // pinned host bytes for spilled checkpoints (0 = automatic: 64 GiB)
     int host_spill = 0;                           // 1: environment checkpoints may live in pinned host memory
     int env_stride = 0;                           // checkpoint spacing of the environment stack (0 = automatic, 1 = keep all)
     double dbss_eps = 0.0;                        // > 0: dynamic block state selection, truncation error target per bond
     int dbss_dmin = 0;                            // DBSS lower bound on the kept states
     int split_k = 0;                              // split-K parts of phase 2 of H_eff psi (0 = automatic)
     int svd_qr = 0;                               // 1: QR-iteration SVD (gesvd) instead of one-sided Jacobi (gesvdj)
+    int eigensolver = 0;                          // 0: Davidson, 1: Lanczos
 };
 struct BondRecord {
     int bond, forward;
@@ -293,6 +294,7 @@ struct Engine {
 // Davidson, decomposition, sweep (sweep.cpp)
 struct DavidsonResult { double theta, residual; int n_matvec; bool converged; double seconds_matvec; };
 DavidsonResult davidson(HeffPlan& p, double* x_dev /*in: guess, out: eigenvector*/, Engine& eng);
+DavidsonResult lanczos(HeffPlan& p, double* x_dev /*in: guess, out: eigenvector*/, Engine& eng);
 void two_site_tensor(const MPS& mps, int i, const HeffPlan& p, double* theta_dev, Engine& eng);
 // SVD + truncation of the two-site vector; replaces sites i, i+1 and bond i+1 of the MPS (reading S14)
 void split_theta(MPS& mps, int i, const HeffPlan& p, const double* theta_dev, int D, bool forward, Engine& eng,

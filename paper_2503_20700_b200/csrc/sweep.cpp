@@ -166,6 +166,99 @@ DavidsonResult davidson(HeffPlan& p, double* x_dev, Engine& eng) {
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// Lanczos (PAPER.md:179 names it beside Davidson; reading S33): full re-orthogonalisation (twice) against the stored
+// Krylov vectors, Rayleigh-Ritz on the tridiagonal matrix, residual norm beta_{m+1} |s_m|, restart from the Ritz vector
+// ---------------------------------------------------------------------------------------------------------------
+DavidsonResult lanczos(HeffPlan& p, double* x_dev, Engine& eng) {
+    const int64_t n = p.nnz;
+    const int maxsub = eng.opt.davidson_max_subspace;
+    cudaStream_t st = eng.stream;
+    DevVec<double> V, w, scal;
+    V.alloc((size_t)maxsub * n); w.alloc((size_t)n);
+    scal.alloc(COMBINE_MAX + 2);
+    std::vector<double> hs((size_t)COMBINE_MAX + 2);
+    auto dots = [&](const double* x, const double* Y, int m) {          // -> hs[0..m)
+        launch_multi_dot(x, Y, n, m, n, scal.p, eng.red_scratch.p, st);
+        eng.launches += 2;
+        cuda_check(cudaMemcpyAsync(hs.data(), scal.p, sizeof(double) * m, cudaMemcpyDeviceToHost, st), "dots");
+        cuda_check(cudaStreamSynchronize(st), "dots");
+    };
+    cudaEvent_t e0, e1;
+    cuda_check(cudaEventCreate(&e0), "event"); cuda_check(cudaEventCreate(&e1), "event");
+    double ms_matvec = 0.0;
+    auto matvec = [&](const double* v, double* y) {
+        cuda_check(cudaEventRecord(e0, st), "event");
+        heff_apply(p, v, y, eng);
+        cuda_check(cudaEventRecord(e1, st), "event");
+        cuda_check(cudaEventSynchronize(e1), "event");
+        float ms = 0.f;
+        cuda_check(cudaEventElapsedTime(&ms, e0, e1), "event");
+        ms_matvec += ms;
+    };
+    dots(x_dev, x_dev, 1);
+    if (!(hs[0] > 0.0)) throw Error(-2, "lanczos: zero initial guess");
+    cuda_check(cudaMemcpyAsync(V.p, x_dev, (size_t)n * 8, cudaMemcpyDeviceToDevice, st), "copy");
+    launch_scale(1.0 / std::sqrt(hs[0]), V.p, n, st); eng.launches++;
+    int m = 1, nmv = 0;
+    std::vector<double> alphas, betas, ev, es, coef(COMBINE_MAX);
+    DavidsonResult res{0.0, 1e300, 0, false, 0.0};
+    for (int iter = 0; iter < eng.opt.davidson_max_iter; ++iter) {
+        double* vlast = V.p + (size_t)(m - 1) * n;
+        matvec(vlast, w.p);
+        ++nmv;
+        dots(w.p, vlast, 1);
+        alphas.push_back(hs[0]);
+        if (m > 1) { const double c[2] = {-betas.back(), -alphas.back()}; launch_combine(w.p, 1.0, V.p + (size_t)(m - 2) * n, n, 2, c, n, st); }
+        else { const double c[1] = {-alphas.back()}; launch_combine(w.p, 1.0, vlast, n, 1, c, n, st); }
+        eng.launches++;
+        for (int gs = 0; gs < 2; ++gs) {
+            dots(w.p, V.p, m);
+            std::vector<double> c(m);
+            for (int i = 0; i < m; ++i) c[i] = -hs[i];
+            launch_combine(w.p, 1.0, V.p, n, m, c.data(), n, st); eng.launches++;
+        }
+        dots(w.p, w.p, 1);
+        const double beta = std::sqrt(std::max(hs[0], 0.0));
+        std::vector<double> T((size_t)m * m, 0.0);
+        for (int i = 0; i < m; ++i) {
+            T[(size_t)i * m + i] = alphas[i];
+            if (i + 1 < m) { T[(size_t)i * m + i + 1] = betas[i]; T[(size_t)(i + 1) * m + i] = betas[i]; }
+        }
+        jacobi_eigh(T, m, ev, es);
+        int lo = 0;
+        for (int i = 1; i < m; ++i) if (ev[i] < ev[lo]) lo = i;
+        for (int i = 0; i < m; ++i) coef[i] = es[(size_t)i * m + lo];
+        const double rn = std::fabs(beta * coef[m - 1]);
+        res.theta = ev[lo]; res.residual = rn; res.n_matvec = nmv;
+        const bool done = rn <= eng.opt.davidson_tol;
+        if (done || beta < 1e-14 || iter + 1 == eng.opt.davidson_max_iter) {
+            res.converged = done;
+            launch_combine(x_dev, 0.0, V.p, n, m, coef.data(), n, st); eng.launches++;
+            dots(x_dev, x_dev, 1);
+            launch_scale(1.0 / std::sqrt(hs[0]), x_dev, n, st); eng.launches++;
+            break;
+        }
+        if (m >= maxsub) {                                                  // restart from the Ritz vector
+            launch_combine(w.p, 0.0, V.p, n, m, coef.data(), n, st); eng.launches++;
+            dots(w.p, w.p, 1);
+            cuda_check(cudaMemcpyAsync(V.p, w.p, (size_t)n * 8, cudaMemcpyDeviceToDevice, st), "copy");
+            launch_scale(1.0 / std::sqrt(hs[0]), V.p, n, st); eng.launches++;
+            m = 1; alphas.clear(); betas.clear();
+            continue;
+        }
+        betas.push_back(beta);
+        cuda_check(cudaMemcpyAsync(V.p + (size_t)m * n, w.p, (size_t)n * 8, cudaMemcpyDeviceToDevice, st), "copy");
+        launch_scale(1.0 / beta, V.p + (size_t)m * n, n, st); eng.launches++;
+        ++m;
+    }
+    cuda_check(cudaStreamSynchronize(st), "lanczos");
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    res.n_matvec = nmv;
+    res.seconds_matvec = ms_matvec * 1e-3;
+    return res;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // theta[l, a, b, r] = sum_m T_i[(l,a)][:, m] T_{i+1}[(m,b)][m, :]      (prediction of the next guess, reading S16)
 // ---------------------------------------------------------------------------------------------------------------
 void two_site_tensor(const MPS& mps, int i, const HeffPlan& p, double* theta_dev, Engine& eng) {
@@ -395,7 +488,7 @@ void Engine::plan_env_policy(int D) {
     // what is free now also has to hold the intermediates of H_eff psi and of the blocking step, the Davidson subspace
     // and the block being grown: the stack gets 55 % of it unless the caller fixes a budget
     const double budget = opt.hbm_budget_bytes > 0 ? (double)opt.hbm_budget_bytes : 0.55 * ((double)free_b + (double)g_device_bytes_env(*this));
-    const double host_budget = opt.host_budget_bytes > 0 ? (double)opt.host_budget_bytes : 96.0 * (double)(1ull << 30);
+    const double host_budget = opt.host_budget_bytes > 0 ? (double)opt.host_budget_bytes : 64.0 * (double)(1ull << 30);
     env_spill = false;
     if (opt.env_stride > 0) { env_stride = opt.env_stride; env_spill = opt.host_spill != 0; return; }
     if (total <= budget) { env_stride = 1; return; }
@@ -510,7 +603,7 @@ static BondRecord optimise(Engine& eng, int i, int D, bool forward) {
     DevVec<double> theta;
     theta.alloc((size_t)p.nnz);
     two_site_tensor(eng.mps, i, p, theta.p, eng);
-    const DavidsonResult dr = davidson(p, theta.p, eng);
+    const DavidsonResult dr = eng.opt.eigensolver == 1 ? lanczos(p, theta.p, eng) : davidson(p, theta.p, eng);
     const auto t2 = clk::now();
     BondRecord rec;
     rec.bond = i; rec.forward = forward ? 1 : 0;

@@ -156,6 +156,10 @@ _CONFIGS = {
     3: dict(name="Fe-S-like CAS(30,20) dense Cholesky", centres=None, D=1024, sweeps=8),
     4: dict(name="circumcoronene CAS(54,54) PPP", centres=lambda: flake_centres(2), D=4096, sweeps=1),
     5: dict(name="icosacene-skeleton CAS(82,82) PPP", centres=lambda: row_centres(20), D=2048, sweeps=1),
+    # not a BASELINE config: the open-shell second workload of SURVEY.md 8(f) rank 4 (Fe-S clusters with
+    # S = 5/2) - the Fe-S-like dense Hamiltonian of config 3 (same recipe, its own seed) with an odd electron count in
+    # the 2Sz = 5 member of a sextet
+    6: dict(name="Fe-S-like open-shell CAS(29,20) dense Cholesky, 2Sz=5", centres=None, D=512, sweeps=4),
 }
 
 
@@ -165,8 +169,10 @@ def make_config(c, rotate=True):
     spec = _CONFIGS[c]
     seed = CONFIG_SEED + c
     rng = np.random.default_rng(seed)
-    if c == 3:
-        k, n_elec = 20, 30
+    two_sz = 0
+    if c in (3, 6):
+        k, n_elec = 20, (30 if c == 3 else 29)
+        two_sz = 0 if c == 3 else 5
         h, eri, e_core = fes_like(k, rng)
         order = np.arange(k)
     else:
@@ -178,5 +184,5 @@ def make_config(c, rotate=True):
             h, eri, _ = rotate_orbitals(h, eri, rng)
         order = fiedler_order(eri)
         h, eri = permute_orbitals(h, eri, order)
-    return dict(name=spec["name"], k=k, n_elec=n_elec, two_sz=0, h=h, eri=eri, e_core=e_core,
+    return dict(name=spec["name"], k=k, n_elec=n_elec, two_sz=two_sz, h=h, eri=eri, e_core=e_core,
                 D=spec["D"], sweeps=spec["sweeps"], seed=seed, order=order)

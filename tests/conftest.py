@@ -20,3 +20,16 @@ def lib():
     g.build()
     import paper_2503_20700_b200 as P
     return P
+
+
+def pytest_addoption(parser):
+    parser.addoption("--runslow", action="store_true", default=False, help="also run the long oracle checks (marker `slow`)")
+
+
+def pytest_collection_modifyitems(config, items):
+    if config.getoption("--runslow") or "slow" in (config.getoption("-m") or ""):
+        return
+    skip = pytest.mark.skip(reason="long oracle check: run with --runslow (or -m slow)")
+    for item in items:
+        if "slow" in item.keywords:
+            item.add_marker(skip)

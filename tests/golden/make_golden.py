@@ -24,6 +24,9 @@ Nothing here imports the CUDA package.  Each file records the command that wrote
   python tests/golden/make_golden.py rdm CFG D
       rdm_cfgC_DD.npz - gamma and Gamma (Eq. 9-10, readings S2 / S20) of random_mps(seed = 900 + CFG,
       gauge R) from oracle.dmrg.rdm12.
+
+CFG 1-5 are BASELINE.json's configs; CFG 6 is the open-shell second workload of synth/ (Fe-S-like CAS(29,20), 2Sz = 5;
+SURVEY.md 8(f) rank 4).
 """
 import json
 import os
@@ -56,7 +59,7 @@ def golden_fci():
 
 def golden_heff(cid, D, bonds):
     cfg = make_config(cid)
-    A, B = dual_gauge_mps(cfg["k"], cfg["n_elec"], 0, D, cfg["seed"] + 2000)
+    A, B = dual_gauge_mps(cfg["k"], cfg["n_elec"], cfg["two_sz"], D, cfg["seed"] + 2000)
     ham = odmrg.Ham(cfg["h"], cfg["eri"])
     t0 = time.time()
     oL = odmrg.build_left(A, ham, max(bonds))
@@ -87,7 +90,7 @@ def golden_heff(cid, D, bonds):
 def golden_sweep(cid, D, nsweeps, Dinit):
     cfg = make_config(cid)
     k, n = cfg["k"], cfg["n_elec"]
-    mps = random_mps(k, n, 0, Dinit, seed=cfg["seed"] + 1000, gauge="R")
+    mps = random_mps(k, n, cfg["two_sz"], Dinit, seed=cfg["seed"] + 1000, gauge="R")
     t0 = time.time()
     eng = odmrg.SweepEngine(cfg["h"], cfg["eri"], mps, davidson_tol=1e-10)
     sweeps = []
@@ -110,7 +113,7 @@ def golden_sweep(cid, D, nsweeps, Dinit):
 def golden_rdm(cid, D):
     cfg = make_config(cid)
     k, n = cfg["k"], cfg["n_elec"]
-    mps = random_mps(k, n, 0, D, seed=900 + cid, gauge="R")
+    mps = random_mps(k, n, cfg["two_sz"], D, seed=900 + cid, gauge="R")
     t0 = time.time()
     g, G = odmrg.rdm12(cfg["h"], cfg["eri"], mps, True)
     note = ("written by `python tests/golden/make_golden.py rdm %d %d` from oracle.dmrg.rdm12; oracle time %.0f s on "

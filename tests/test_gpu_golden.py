@@ -25,7 +25,7 @@ def test_golden_files_present():
     """configs 4 and 5 must have an H_eff golden, configs 2 and 3 a sweep and an RDM golden."""
     for c in (4, 5):
         assert _files("heff_cfg%d_D*.npz" % c)
-    for c in (2, 3):
+    for c in (2, 3, 6):                                           # 6: the open-shell second workload (2Sz = 5, odd N)
         assert _files("sweep_cfg%d_D*.json" % c) and _files("rdm_cfg%d_D*.npz" % c)
 
 
@@ -35,11 +35,12 @@ def test_heff_vs_golden(lib, name):
     cid, D = int(z["config"]), int(z["D"])
     cfg = make_config(cid)
     k, n = cfg["k"], cfg["n_elec"]
-    A, B = dual_gauge_mps(k, n, 0, D, int(z["mps_seed"]))
-    ctx = lib.dmrg_create(k, n, 0, cfg["h"], cfg["eri"], keep_env_stack=0)
+    s2 = cfg["two_sz"]
+    A, B = dual_gauge_mps(k, n, s2, D, int(z["mps_seed"]))
+    ctx = lib.dmrg_create(k, n, s2, cfg["h"], cfg["eri"], keep_env_stack=0)
     try:
         for i in [int(b) for b in z["bonds"]]:
-            lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mixed_gauge(A, B, i)), k, n, 0)
+            lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mixed_gauge(A, B, i)), k, n, s2)
             lib.dmrg_prepare_bond(ctx, i)
             nnz, lay = lib.dmrg_heff_layout(ctx, i)
             assert nnz == int(z["nnz_%d" % i])
@@ -67,11 +68,11 @@ def test_heff_vs_golden(lib, name):
 def test_sweep_vs_golden(lib, name):
     gold = json.load(open(os.path.join(GOLD, name)))
     cfg = make_config(gold["config"])
-    k, n, D = cfg["k"], cfg["n_elec"], gold["D"]
-    mps = random_mps(k, n, 0, gold["Dinit"], seed=gold["mps_seed"], gauge="R")
-    ctx = lib.dmrg_create(k, n, 0, cfg["h"], cfg["eri"], davidson_tol=gold["davidson_tol"])
+    k, n, s2, D = cfg["k"], cfg["n_elec"], cfg["two_sz"], gold["D"]
+    mps = random_mps(k, n, s2, gold["Dinit"], seed=gold["mps_seed"], gauge="R")
+    ctx = lib.dmrg_create(k, n, s2, cfg["h"], cfg["eri"], davidson_tol=gold["davidson_tol"])
     try:
-        lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, 0)
+        lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, s2)
         for s, gs in enumerate(gold["sweeps"]):
             r = lib.dmrg_sweep(ctx, D, k)
             assert abs(r["energy_last"] - gs["energy_last"]) <= 1e-8
@@ -91,11 +92,11 @@ def test_rdm_vs_golden(lib, name):
     z = np.load(os.path.join(GOLD, name), allow_pickle=False)
     cid, D = int(z["config"]), int(z["D"])
     cfg = make_config(cid)
-    k, n = cfg["k"], cfg["n_elec"]
-    mps = random_mps(k, n, 0, D, seed=int(z["mps_seed"]), gauge="R")
-    ctx = lib.dmrg_create(k, n, 0, cfg["h"], cfg["eri"])
+    k, n, s2 = cfg["k"], cfg["n_elec"], cfg["two_sz"]
+    mps = random_mps(k, n, s2, D, seed=int(z["mps_seed"]), gauge="R")
+    ctx = lib.dmrg_create(k, n, s2, cfg["h"], cfg["eri"])
     try:
-        lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, 0)
+        lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, s2)
         g, G = lib.dmrg_rdm12(ctx, k, True)
     finally:
         lib.dmrg_destroy(ctx)

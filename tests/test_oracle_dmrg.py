@@ -7,12 +7,15 @@ from oracle import fci, dmrg
 from synth import random_dense, random_mps, make_config, full_sector_dims
 
 
-@pytest.mark.parametrize("k,n,s2,D", [(4, 4, 0, 8), (5, 5, 1, 10), (6, 8, 0, 12), (6, 3, -1, 12)])
-def test_heff_vs_bruteforce_every_bond(k, n, s2, D):
+@pytest.mark.parametrize("k,n,s2,D,bonds", [
+    (4, 4, 0, 8, None), (5, 5, 1, 10, None), (6, 8, 0, 12, None), (6, 3, -1, 12, None),
+    (8, 8, 0, 16, (0, 3, 6)),                                           # k = 8: both ends and the middle
+    pytest.param(10, 10, 0, 20, (4,), marks=pytest.mark.slow)])        # k = 10 (FCI dimension 63504), mid-chain
+def test_heff_vs_bruteforce_every_bond(k, n, s2, D, bonds):
     h, eri = random_dense(k, 40 + k)
     ham = dmrg.Ham(h, eri)
     sp = fci.FCISpace(k, n, s2)
-    for i in range(k - 1):
+    for i in (range(k - 1) if bonds is None else bonds):
         mps = random_mps(k, n, s2, D, seed=70 + i, gauge="LR:%d" % i)
         L = dmrg.build_left(mps, ham, i)[-1]
         R = dmrg.build_right(mps, ham, i + 2)[i + 2]
@@ -176,3 +179,111 @@ def test_dbss_sweep_truncation_error_below_target():
     for _ in range(3):
         e_lo, e_hi = lo.sweep(dmin)["energy_last"], hi.sweep(dmax)["energy_last"]
     assert e_hi - 1e-9 <= r["energy_last"] <= e_lo + 1e-9
+
+
+def _jw_dense(k):
+    """Dense Jordan-Wigner annihilators a_P on the 4^k Fock space, site 0 slowest, local order (|0>,|dn>,|up>,|up dn>),
+    spin orbital P = 2p + [dn]: a_P = F x ... x F x a_local x 1 x ... x 1 (F = (-1)^N of the sites before p)."""
+    F = np.diag([1.0, -1.0, -1.0, 1.0])
+    out = []
+    for P in range(2 * k):
+        m = np.ones((1, 1))
+        for q in range(k):
+            m = np.kron(m, F if q < P // 2 else (dmrg.site_ann(P) if q == P // 2 else np.eye(4)))
+        out.append(m)
+    return out
+
+
+def test_block_operators_are_projected_jordan_wigner_matrices():
+    """Operator identities against dense Jordan-Wigner matrices (k = 3): every stored operator of a renormalised left
+    block equals V^T O V, with O the dense operator built from its DEFINITION (C3 step 1: a+_P, A_PQ = a+_P a+_Q,
+    B_PS = a+_P a_S, H_X, S_P^X) on the block's own Fock space and V the isometry the site tensors define (Eq. 14)."""
+    k, n, s2, nb = 3, 3, 1, 2
+    h, eri = random_dense(k, 11)
+    ham = dmrg.Ham(h, eri)
+    mps = random_mps(k, n, s2, 16, seed=4, gauge="L")
+    blk = dmrg.build_left(mps, ham, nb)[-1]
+    # isometry V [4^nb, dim(bond nb)]: V[(s0 s1), (sector, alpha)] = (A0[s0] A1[s1])[0, alpha]
+    cols = []
+    for ri, (N, S, d) in enumerate(blk.basis):
+        V = np.zeros((4 ** nb, d))
+        for s0 in range(4):
+            for s1 in range(4):
+                t0 = mps["tensors"][0].get((0, s0))
+                if t0 is None:
+                    continue
+                n1, z1 = dmrg.SITE_Q[s0]
+                mid = [j for j, (a, b, _) in enumerate(mps["bonds"][1]) if (a, b) == (n1, z1)]
+                if not mid:
+                    continue
+                t1 = mps["tensors"][1].get((mid[0], s1))
+                if t1 is None or (n1 + dmrg.SITE_Q[s1][0], z1 + dmrg.SITE_Q[s1][1]) != (N, S):
+                    continue
+                V[s0 * 4 + s1] = (t0 @ t1)[0]
+        cols.append(V)
+    a = _jw_dense(nb)                                                   # operators of the block's own sites
+    ad = [m.T for m in a]
+    inside = list(range(2 * nb))
+
+    def check(op, dense):
+        for i, (N, S, d) in enumerate(blk.basis):
+            for o in range(len(blk.basis)):
+                ref = cols[o].T @ dense @ cols[i]
+                if i in op.blocks and op.blocks[i][0] == o:
+                    assert np.abs(op.blocks[i][1] - ref).max() < 1e-12
+                else:
+                    assert np.abs(ref).max() < 1e-12
+
+    for P in inside:
+        check(blk.ops[("C", P)], ad[P])
+        for Q in inside:
+            if P < Q:
+                check(blk.ops[("A", P, Q)], ad[P] @ ad[Q])
+            check(blk.ops[("B", P, Q)], ad[P] @ a[Q])
+    Hd = sum(ham.t(P, Q) * ad[P] @ a[Q] for P in inside for Q in inside)
+    Hd = Hd + 0.5 * sum(ham.v(P, Q, R, S) * ad[P] @ ad[Q] @ a[R] @ a[S]
+                        for P in inside for Q in inside for R in inside for S in inside)
+    check(blk.ops[("H",)], Hd)
+    for P in range(2 * nb, 2 * k):                                      # S_P^X for P outside, by definition
+        Sd = sum(0.5 * ham.t(P, Q) * a[Q] for Q in inside)
+        Sd = Sd + sum(ham.v(P, Q, R, S) * ad[Q] @ a[R] @ a[S] for Q in inside for R in inside for S in inside)
+        check(blk.ops[("S", P)], Sd)
+
+
+def test_lanczos_against_dense_eigh_and_davidson():
+    """Lanczos reaches the lowest eigenpair of a dense symmetric matrix (numpy eigh), through restarts,
+    and agrees with Davidson on an H_eff."""
+    rng = np.random.default_rng(8)
+    n = 300
+    M = rng.normal(size=(n, n))
+    M = M + M.T + np.diag(np.arange(n) * 1.5)
+    w = np.linalg.eigvalsh(M)
+    for sub in (40, 8):                                                  # without and with restarts
+        th, u, nmv, rn, ok = dmrg.lanczos(lambda v: M @ v, rng.normal(size=n), tol=1e-10, max_iter=2000, max_subspace=sub)
+        assert ok and abs(th - w[0]) < 1e-10 and np.linalg.norm(M @ u - th * u) < 1e-9
+    k, n_e, s2, i = 6, 6, 0, 2
+    h, eri = random_dense(k, 3)
+    ham = dmrg.Ham(h, eri)
+    mps = random_mps(k, n_e, s2, 8, seed=1, gauge="LR:%d" % i)
+    H = dmrg.Heff(dmrg.build_left(mps, ham, i)[-1], dmrg.build_right(mps, ham, i + 2)[i + 2], ham, i)
+    x0 = rng.normal(size=H.nnz)
+    t1 = dmrg.lanczos(H.apply, x0, tol=1e-11, max_iter=500)
+    t2 = dmrg.davidson(H.apply, H.diagonal(), x0, tol=1e-11, max_iter=500)
+    assert t1[4] and t2[4] and abs(t1[0] - t2[0]) < 1e-10 and abs(abs(t1[1] @ t2[1]) - 1.0) < 1e-9
+
+
+def test_sweep_stopping_rule():
+    """eps_sweep rule (reading S34) on hand-made energy sequences, and inside SweepEngine.solve."""
+    conv = dmrg.sweeps_converged
+    assert not conv([-1.0, -1.0], 1e-3)                                  # needs three sweeps
+    assert conv([-1.0, -1.0004, -1.0007], 1e-3)
+    assert not conv([-1.0, -1.002, -1.0021], 1e-3)                       # first difference too large
+    assert not conv([-1.0, -1.0001, -1.002], 1e-3)                       # second difference too large
+    assert conv([-0.5, -1.0, -1.0004, -1.0007], 1e-3)                    # only the last three count
+    k, n, s2 = 6, 6, 0
+    h, eri = random_dense(k, 9)
+    mps = random_mps(k, n, s2, 16, seed=2, gauge="R")
+    eng = dmrg.SweepEngine(h, eri, mps, davidson_tol=1e-9)
+    out = eng.solve(16, 1e-6, 12)
+    e = [r["energy_last"] for r in out]
+    assert 3 <= len(e) < 12 and conv(e, 1e-6) and not any(conv(e[:j], 1e-6) for j in range(len(e)))
