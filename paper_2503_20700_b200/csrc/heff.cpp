@@ -74,9 +74,9 @@ static std::vector<NTerm> heff_terms(const Ham& ham, Block& LB, Block& RB, const
         for (int P : A)                                        // B_PS^A Q_PS^Y
             for (int S : A)
                 for (Term t : gen.B(P, S)) { t.f.push_back(yf(L2(K_Q, P, S), false)); T.push_back(t); }
-    std::vector<NTerm> out;
-    out.reserve(T.size());
-    for (const Term& t : T) out.push_back(normalise(t, "LdR", dot));
+    std::vector<NTerm> out(T.size());                          // 16 x 16 dot-matrix products per term: host threads
+#pragma omp parallel for schedule(static, 64)
+    for (long j = 0; j < (long)T.size(); ++j) out[j] = normalise(T[j], "LdR", dot);
     return out;
 }
 

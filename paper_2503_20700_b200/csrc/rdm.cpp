@@ -28,6 +28,8 @@
 #include <cmath>
 #include <cstring>
 
+#include <omp.h>
+
 #include "core.hpp"
 
 namespace dmrg {
@@ -510,32 +512,53 @@ void move_centre_right(const SiteTensor& psi, const Basis& bl, const Basis& br, 
     if (next.nnz) cuda_check(cudaMemsetAsync(next.data.p, 0, (size_t)next.nnz * 8, st), "memset");
     std::vector<DevVec<double>> rms(br.size());
     GemmBatch gb;
+    // sector SVDs concurrently: a few host threads, each with its own stream and cuSOLVER handle (psi is complete: the
+    // previous step ended synchronised)
+    cuda_check(cudaStreamSynchronize(st), "rdm centre move");
+    const int nthreads = 4;
+    eng.ensure_svd_pool(nthreads);
+    std::string err;
+    int64_t nlaunch = 0;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads) reduction(+ : nlaunch)
     for (int r = 0; r < (int)br.size(); ++r) {
-        std::vector<const SiteTensor::Blk*> rows;
-        int mrows = 0;
-        for (const auto& b : psi.blocks) if (b.r == r) { rows.push_back(&b); mrows += b.rows; }
+        try {
+            const int tid = omp_get_thread_num();
+            cudaStream_t ts = eng.svd_streams[tid];
+            cuda_check(cudaSetDevice(eng.opt.device_id), "cudaSetDevice");
+            std::vector<const SiteTensor::Blk*> rows;
+            int mrows = 0;
+            for (const auto& b : psi.blocks) if (b.r == r) { rows.push_back(&b); mrows += b.rows; }
+            const int n = br[r].d;
+            if (mrows < n) throw Error(-2, "rdm12: rank-deficient centre (bond sector wider than its left space)");
+            DevVec<double> buf, U, S, Vt;
+            buf.alloc((size_t)mrows * n); U.alloc((size_t)mrows * n); S.alloc((size_t)n); Vt.alloc((size_t)n * n);
+            int off = 0;
+            for (const auto* b : rows) {
+                launch_copy2d(buf.p + (size_t)off * n, n, b->ptr, b->ld, b->rows, n, 1.0, nullptr, nullptr, ts);
+                nlaunch++;
+                off += b->rows;
+            }
+            svd_rowmajor(eng.svd_pool[tid], buf.p, mrows, n, U.p, S.p, Vt.p, ts);
+            off = 0;
+            for (const auto* b : rows) {
+                const SiteTensor::Blk* ab = A.get(b->l, b->s);
+                launch_copy2d(ab->ptr, ab->ld, U.p + (size_t)off * n, n, b->rows, n, 1.0, nullptr, nullptr, ts);
+                nlaunch++;
+                off += b->rows;
+            }
+            rms[r].alloc((size_t)n * n);
+            launch_copy2d(rms[r].p, n, Vt.p, n, n, n, 1.0, S.p, nullptr, ts);
+            nlaunch++;
+            cuda_check(cudaStreamSynchronize(ts), "rdm centre move");      // buf / U / S / Vt die here
+        } catch (const std::exception& e) {
+#pragma omp critical
+            err = e.what();
+        }
+    }
+    if (!err.empty()) throw Error(-2, err);
+    eng.launches += nlaunch;
+    for (int r = 0; r < (int)br.size(); ++r) {
         const int n = br[r].d;
-        if (mrows < n) throw Error(-2, "rdm12: rank-deficient centre (bond sector wider than its left space)");
-        DevVec<double> buf, U, S, Vt;
-        buf.alloc((size_t)mrows * n); U.alloc((size_t)mrows * n); S.alloc((size_t)n); Vt.alloc((size_t)n * n);
-        int off = 0;
-        for (const auto* b : rows) {
-            launch_copy2d(buf.p + (size_t)off * n, n, b->ptr, b->ld, b->rows, n, 1.0, nullptr, nullptr, st);
-            eng.launches++;
-            off += b->rows;
-        }
-        svd_rowmajor(eng.svd, buf.p, mrows, n, U.p, S.p, Vt.p, st);
-        off = 0;
-        for (const auto* b : rows) {
-            const SiteTensor::Blk* ab = A.get(b->l, b->s);
-            launch_copy2d(ab->ptr, ab->ld, U.p + (size_t)off * n, n, b->rows, n, 1.0, nullptr, nullptr, st);
-            eng.launches++;
-            off += b->rows;
-        }
-        rms[r].alloc((size_t)n * n);
-        launch_copy2d(rms[r].p, n, Vt.p, n, n, n, 1.0, S.p, nullptr, st);
-        eng.launches++;
-        cuda_check(cudaStreamSynchronize(st), "rdm centre move");      // buf / U / S / Vt die here
         for (int s = 0; s < 4; ++s) {
             const SiteTensor::Blk* nb = next.get(r, s);
             if (!nb) continue;
@@ -560,32 +583,51 @@ void move_centre_left(const SiteTensor& psi, const Basis& bl, const Basis& br, c
     if (prev.nnz) cuda_check(cudaMemsetAsync(prev.data.p, 0, (size_t)prev.nnz * 8, st), "memset");
     std::vector<DevVec<double>> lms(bl.size());
     GemmBatch gb;
+    cuda_check(cudaStreamSynchronize(st), "rdm centre move");
+    const int nthreads = 4;
+    eng.ensure_svd_pool(nthreads);
+    std::string err;
+    int64_t nlaunch = 0;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads) reduction(+ : nlaunch)
     for (int l = 0; l < (int)bl.size(); ++l) {
-        std::vector<const SiteTensor::Blk*> cols;
-        int ncols = 0;
-        for (const auto& b : psi.blocks) if (b.l == l) { cols.push_back(&b); ncols += b.cols; }
+        try {
+            const int tid = omp_get_thread_num();
+            cudaStream_t ts = eng.svd_streams[tid];
+            cuda_check(cudaSetDevice(eng.opt.device_id), "cudaSetDevice");
+            std::vector<const SiteTensor::Blk*> cols;
+            int ncols = 0;
+            for (const auto& b : psi.blocks) if (b.l == l) { cols.push_back(&b); ncols += b.cols; }
+            const int m = bl[l].d;
+            if (ncols < m) throw Error(-2, "rdm12: rank-deficient centre (bond sector wider than its right space)");
+            DevVec<double> buf, U, S, Vt;
+            buf.alloc((size_t)m * ncols); U.alloc((size_t)m * m); S.alloc((size_t)m); Vt.alloc((size_t)m * ncols);
+            int off = 0;
+            for (const auto* b : cols) {
+                launch_copy2d(buf.p + off, ncols, b->ptr, b->ld, m, b->cols, 1.0, nullptr, nullptr, ts);
+                nlaunch++;
+                off += b->cols;
+            }
+            svd_rowmajor(eng.svd_pool[tid], buf.p, m, ncols, U.p, S.p, Vt.p, ts);
+            off = 0;
+            for (const auto* b : cols) {
+                const SiteTensor::Blk* bb = B.get(b->l, b->s);
+                launch_copy2d(bb->ptr, bb->ld, Vt.p + off, ncols, m, b->cols, 1.0, nullptr, nullptr, ts);
+                nlaunch++;
+                off += b->cols;
+            }
+            lms[l].alloc((size_t)m * pad2(m));
+            launch_copy2d(lms[l].p, pad2(m), U.p, m, m, m, 1.0, nullptr, S.p, ts);   // Lm = U diag(S)
+            nlaunch++;
+            cuda_check(cudaStreamSynchronize(ts), "rdm centre move");      // buf / U / S / Vt die here
+        } catch (const std::exception& e) {
+#pragma omp critical
+            err = e.what();
+        }
+    }
+    if (!err.empty()) throw Error(-2, err);
+    eng.launches += nlaunch;
+    for (int l = 0; l < (int)bl.size(); ++l) {
         const int m = bl[l].d;
-        if (ncols < m) throw Error(-2, "rdm12: rank-deficient centre (bond sector wider than its right space)");
-        DevVec<double> buf, U, S, Vt;
-        buf.alloc((size_t)m * ncols); U.alloc((size_t)m * m); S.alloc((size_t)m); Vt.alloc((size_t)m * ncols);
-        int off = 0;
-        for (const auto* b : cols) {
-            launch_copy2d(buf.p + off, ncols, b->ptr, b->ld, m, b->cols, 1.0, nullptr, nullptr, st);
-            eng.launches++;
-            off += b->cols;
-        }
-        svd_rowmajor(eng.svd, buf.p, m, ncols, U.p, S.p, Vt.p, st);
-        off = 0;
-        for (const auto* b : cols) {
-            const SiteTensor::Blk* bb = B.get(b->l, b->s);
-            launch_copy2d(bb->ptr, bb->ld, Vt.p + off, ncols, m, b->cols, 1.0, nullptr, nullptr, st);
-            eng.launches++;
-            off += b->cols;
-        }
-        lms[l].alloc((size_t)m * pad2(m));
-        launch_copy2d(lms[l].p, pad2(m), U.p, m, m, m, 1.0, nullptr, S.p, st);   // Lm = U diag(S)
-        eng.launches++;
-        cuda_check(cudaStreamSynchronize(st), "rdm centre move");      // buf / U / S / Vt die here
         for (const auto& ab : aprev.blocks) {
             if (ab.r != l) continue;
             const SiteTensor::Blk* pb = prev.get(ab.l, ab.s);
