@@ -57,6 +57,11 @@ typedef struct dmrg_options {
     int32_t host_maps;            /* default 0: block maps built on the device; 1: host reference builder (A/B tests)  */
     int32_t generic_gemm;         /* default 0; 1: always the cp.async GEMM kernel instead of the bulk-copy one (A/B)  */
     int32_t eigensolver;          /* default 0: Davidson; 1: Lanczos (PAPER.md:179 names both); same tolerance fields  */
+    int32_t rdm_split;            /* default -1 = k/2: site kh of the half-chain partition of dmrg_rdm12 (strings with their
+                                     third-smallest site < kh are evaluated there with the two-index operators on the left,
+                                     the others at their second-smallest site with them on the right); 0 and k give the two
+                                     one-sided evaluation orders.  Results do not depend on it (tested); memory does.       */
+    int32_t reserved0;
 } dmrg_options;
 
 /* Neutral MPS exchange format (host memory, caller-owned, flat arrays).

@@ -28,7 +28,8 @@ class dmrg_options(C.Structure):
                 ("keep_env_stack", C.c_int32), ("workspace_bytes", C.c_int64),
                 ("hbm_budget_bytes", C.c_int64), ("host_budget_bytes", C.c_int64), ("host_spill", C.c_int32),
                 ("env_stride", C.c_int32), ("dbss_eps", C.c_double), ("dbss_dmin", C.c_int32), ("split_k", C.c_int32),
-                ("svd_qr", C.c_int32), ("host_maps", C.c_int32), ("generic_gemm", C.c_int32), ("eigensolver", C.c_int32)]
+                ("svd_qr", C.c_int32), ("host_maps", C.c_int32), ("generic_gemm", C.c_int32), ("eigensolver", C.c_int32),
+                ("rdm_split", C.c_int32), ("reserved0", C.c_int32)]
 
 
 class dmrg_mps_blob(C.Structure):

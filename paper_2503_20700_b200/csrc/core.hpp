@@ -230,6 +230,7 @@ struct Options {
     int split_k = 0;                              // split-K parts of phase 2 of H_eff psi (0 = automatic)
     int svd_qr = 0;                               // 1: QR-iteration SVD (gesvd) instead of one-sided Jacobi (gesvdj)
     int eigensolver = 0;                          // 0: Davidson, 1: Lanczos
+    int rdm_split = -1;                           // site kh separating the two centre rules of the RDM pass (-1: k/2)
 };
 struct BondRecord {
     int bond, forward;

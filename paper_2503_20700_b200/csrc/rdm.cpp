@@ -663,7 +663,8 @@ void add_identity(Block& b, Engine& eng) {
 
 void rdm12(Engine& eng, double* gamma, double* Gamma) {
     const double t_begin = now_s();
-    const int k = eng.k, kh = k / 2;
+    const int k = eng.k;
+    const int kh = (eng.opt.rdm_split >= 0 && eng.opt.rdm_split <= k) ? eng.opt.rdm_split : k / 2;   // partition point of the two rules
     const bool want2 = Gamma != nullptr;
     MPS& mps = eng.mps;
     for (int p = 1; p < k; ++p)

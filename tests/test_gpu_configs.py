@@ -156,3 +156,34 @@ def test_config5_D1024_properties(lib):
         assert 0 < st["f_exec"] <= st["f_alg"] and st["nterms"] > 13000
     finally:
         lib.dmrg_destroy(ctx)
+
+
+def test_config4_reduced_D_sweep_memory_path_and_rdm(lib):
+    """BASELINE config 4 (k = 54) at D = 96: one sweep with every environment block resident against the same sweep
+    under a device budget that forces checkpoints, recomputation and the pinned-host spill (bit-identical), then the
+    RDM pass on the swept MPS: E_RDM = <Psi|H|Psi> must equal the last Davidson Rayleigh quotient up to the truncation of
+    the final bond (reading S20), Tr gamma = N, partial trace."""
+    cfg = make_config(4)
+    k, n, D = cfg["k"], cfg["n_elec"], 96
+    mps = random_mps(k, n, 0, D, seed=cfg["seed"] + 1000, gauge="R")
+    out = []
+    for opts in (dict(env_stride=1), dict(hbm_budget_bytes=60 << 20, host_budget_bytes=40 << 20, host_spill=1)):
+        ctx = lib.dmrg_create(k, n, 0, cfg["h"], cfg["eri"], davidson_max_iter=6, **opts)
+        try:
+            lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, 0)
+            r = lib.dmrg_sweep(ctx, D, k)
+            st = lib.dmrg_sweep_stats(ctx)
+            g, G = lib.dmrg_rdm12(ctx, k, True) if not out else (None, None)
+            out.append((r, st, g, G))
+        finally:
+            lib.dmrg_destroy(ctx)
+    (ra, sa, g, G), (rb, sb, _, _) = out
+    assert sa["env_stride"] == 1 and sa["host_spill"] == 0
+    assert sb["env_stride"] > 1 and sb["host_spill"] == 1 and sb["bytes_spilled"] > 0 and sb["seconds_regrow"] > 0
+    assert [b["energy"] for b in ra["bonds"]] == [b["energy"] for b in rb["bonds"]]
+    assert [b["kept"] for b in ra["bonds"]] == [b["kept"] for b in rb["bonds"]]
+    assert abs(np.trace(g) - n) <= 1e-9
+    assert np.abs(np.einsum("pqrr->pq", G) - (n - 1) * g).max() <= 1e-8
+    e_rdm = np.einsum("pq,pq->", cfg["h"], g) + 0.5 * np.einsum("pqrs,pqrs->", cfg["eri"], G)
+    last = ra["bonds"][-1]
+    assert abs(e_rdm - last["energy"]) <= 1e-6 + 10 * last["trunc_err"]   # Davidson capped at 6 iterations: Rayleigh quotient of the kept state

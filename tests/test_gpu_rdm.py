@@ -129,3 +129,41 @@ def test_rdm12_config_geometries_small_D_vs_oracle(lib, cid, D):
         lib.dmrg_destroy(ctx)
     assert np.abs(g - g0).max() <= TOL and np.abs(G - G0).max() <= TOL
     _invariants(g, G, n)
+
+
+@pytest.mark.parametrize("k,n,s2,D", [(6, 6, 0, 12), (7, 8, 2, 16), (8, 7, 1, 20)])
+def test_rdm12_partition_point_does_not_matter_and_matches_oracle(lib, k, n, s2, D):
+    """Half-chain partition: every partition point kh = 0 (right rule only: c = s2, two-index operators on
+    the right - the oracle's order), k (left rule only: c = s3, on the left - the round-1 order) and everything between
+    gives the oracle's RDMs."""
+    h, eri = random_dense(k, 700 + k)
+    mps = random_mps(k, n, s2, D, seed=80 + k, gauge="R")
+    g0, G0 = odmrg.rdm12(h, eri, mps, True)
+    for kh in [0, 1, k // 2, k - 1, k, -1]:
+        ctx = lib.dmrg_create(k, n, s2, h, eri, rdm_split=kh)
+        try:
+            lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, s2)
+            g, G = lib.dmrg_rdm12(ctx, k, True)
+        finally:
+            lib.dmrg_destroy(ctx)
+        assert np.abs(g - g0).max() <= TOL and np.abs(G - G0).max() <= TOL, kh
+
+
+def test_rdm12_config4_chain_partition_points_agree(lib):
+    """BASELINE config 4 (k = 54, the 9 279-term Hamiltonian) at reduced D: the pass with the partition in the middle
+    (the one that scales) against the two one-sided evaluation orders, which the oracle tests above pin; invariants."""
+    cfg = make_config(4)
+    k, n, D = cfg["k"], cfg["n_elec"], 48
+    mps = random_mps(k, n, 0, D, seed=4321, gauge="R")
+    res = []
+    for kh in (-1, 0, k):
+        ctx = lib.dmrg_create(k, n, 0, cfg["h"], cfg["eri"], rdm_split=kh)
+        try:
+            lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, 0)
+            res.append(lib.dmrg_rdm12(ctx, k, True))
+        finally:
+            lib.dmrg_destroy(ctx)
+    (g, G) = res[0]
+    for (g1, G1) in res[1:]:
+        assert np.abs(g - g1).max() <= TOL and np.abs(G - G1).max() <= TOL
+    _invariants(g, G, n)
