@@ -71,6 +71,7 @@ def parse_args():
     ap.add_argument("--sample-D", type=int, default=48, help="bond dimension of the oracle's bounded sample")
     ap.add_argument("--sweep-D", type=int, default=2048, help="bond dimension of the --big sweeps")
     ap.add_argument("--workspace-gb", type=float, default=0.0, help="intermediate workspace of H_eff psi (0 = library default)")
+    ap.add_argument("--split-k", type=int, default=0, help="split-K parts of phase 2 of H_eff psi (0 = library default)")
     ap.add_argument("--probe", type=int, default=1, help="1: run the FP64 ceiling probes (DMMA, DFMA, LDS-fed DMMA, cuBLAS DGEMM)")
     return ap.parse_args()
 
@@ -312,6 +313,10 @@ def time_small_extras(P, torch, peaks, level):
     out = {}
     for cid, nsweep in [(1, 3), (2, 1), (3, 1)][: 1 if level == 1 else 3]:
         out["config%d" % cid] = time_sweep_rdm(P, torch, peaks, cid, {1: 64, 2: 512, 3: 1024}[cid], nsweep)
+    if level >= 2:
+        # the RDM pass at the metric's chain length (k = 54, half-chain partition) on the seeded random MPS at D = 1024; the
+        # sweeps of config 4 (105 / 320 s at D = 1024 / 2048) are `--big 4` runs, profiles/r02_big_cfg4_*
+        out["config4_rdm"] = time_sweep_rdm(P, torch, peaks, 4, 1024, 0)
     return out
 
 
@@ -361,7 +366,7 @@ def run_ours(args):
     cfg, D, i, mps, blob = build_workload(args.config, args.D, args.bond)
     k, n = cfg["k"], cfg["n_elec"]
     ctx = P.dmrg_create(k, n, 0, cfg["h"], cfg["eri"], keep_env_stack=0, device_id=local_rank,
-                        workspace_bytes=int(args.workspace_gb * (1 << 30)))
+                        workspace_bytes=int(args.workspace_gb * (1 << 30)), split_k=args.split_k)
     P.dmrg_mps_import(ctx, blob, k, n, 0)
     t_env = time.perf_counter()
     f_env = P.dmrg_flops_total(ctx)

@@ -52,7 +52,7 @@ typedef struct dmrg_options {
      * whose discarded weight is <= dbss_eps, at least dbss_dmin and at most the D passed to dmrg_sweep (D_max).       */
     double dbss_eps;              /* default 0 = fixed D                                                               */
     int32_t dbss_dmin;            /* default 0                                                                         */
-    int32_t split_k;              /* default 0 = automatic: split-K parts (1..16) of phase 2 of H_eff psi              */
+    int32_t split_k;              /* default 0 = automatic: split-K parts (1..64) of phase 2 of H_eff psi              */
     int32_t svd_qr;               /* default 0: one-sided Jacobi SVD (cuSOLVER gesvdj, gesvd fallback); 1: gesvd       */
     int32_t host_maps;            /* default 0: block maps built on the device; 1: host reference builder (A/B tests)  */
     int32_t generic_gemm;         /* default 0; 1: always the cp.async GEMM kernel instead of the bulk-copy one (A/B)  */

@@ -4,6 +4,8 @@
 #include <cstdlib>
 #include <cstring>
 
+#include <omp.h>
+
 #include "../../include/dmrg_b200.h"
 #include "core.hpp"
 
@@ -113,7 +115,7 @@ int dmrg_create(dmrg_ctx** out, int k, int n_elec, int two_sz, const double* h, 
         }
         if (eng.opt.davidson_max_subspace < 2 || eng.opt.davidson_max_subspace > COMBINE_MAX ||
             eng.opt.davidson_max_iter < 1 || !(eng.opt.davidson_tol > 0) || eng.opt.env_stride < 0 ||
-            eng.opt.split_k < 0 || eng.opt.split_k > 16 || eng.opt.dbss_eps < 0 || eng.opt.dbss_dmin < 0 ||
+            eng.opt.split_k < 0 || eng.opt.split_k > 64 || eng.opt.dbss_eps < 0 || eng.opt.dbss_dmin < 0 ||
             eng.opt.hbm_budget_bytes < 0 || eng.opt.host_budget_bytes < 0 || eng.opt.eigensolver < 0 ||
             eng.opt.eigensolver > 1) { delete ctx; return DMRG_EINVAL; }
         int ndev = 0;
@@ -127,6 +129,8 @@ int dmrg_create(dmrg_ctx** out, int k, int n_elec, int two_sz, const double* h, 
         eng.ham.k = k;
         eng.ham.h.assign(h, h + (size_t)k * k);
         eng.ham.eri.assign(eri, eri + (size_t)k * k * k * k);
+        eng.host_threads = std::max(1, std::min(8, omp_get_num_procs()));
+        omp_set_num_threads(eng.host_threads);
         eng.svd = svd_create(eng.stream, eng.opt.svd_qr == 0);
         eng.red_scratch.alloc((size_t)multi_dot_scratch());
         { const char* g = std::getenv("DMRG_B200_TRACE"); eng.trace = g && g[0] == '1'; }   // diagnostics only: per-launch times on stderr

@@ -109,7 +109,7 @@ void finalize(GemmBatch& b, GemmLaunch& out, Engine& eng) {
     std::vector<double> weight(nt, 0.0);
     std::vector<int> ntile((size_t)nt + 1, 0);
     int aligned_i = 1;
-#pragma omp parallel for schedule(static, 256) reduction(&& : aligned_i)
+#pragma omp parallel for schedule(static, 256) reduction(&& : aligned_i) if (nt > 4096)
     for (int t = 0; t < nt; ++t) {
         int* v0 = idx.data() + off[t];
         int* v1 = idx.data() + off[t + 1];
@@ -155,7 +155,7 @@ void finalize(GemmBatch& b, GemmLaunch& out, Engine& eng) {
     const size_t ntl = (size_t)ntile[nt];
     std::vector<Tile> raw(ntl);
     std::vector<double> tw(ntl);
-#pragma omp parallel for schedule(static, 256)
+#pragma omp parallel for schedule(static, 256) if (nt > 4096)
     for (int t = 0; t < nt; ++t) {
         const Task& tk = b.tasks[t];
         if (tk.M <= 0 || tk.N <= 0) continue;

@@ -257,6 +257,8 @@ struct Engine {
     std::vector<SvdWork*> svd_pool;               // extra cuSOLVER handles on their own streams: sector SVDs run concurrently
     std::vector<cudaStream_t> svd_streams;
     void ensure_svd_pool(int n);
+    int host_threads = 1;                         // size of the one OpenMP team every host-parallel region uses (a changing
+                                                  // team size makes libgomp rebuild its thread pool at every region)
     double rdm_seconds = 0, rdm_bytes = 0, rdm_flops = 0, rdm_host_seconds = 0, rdm_grow_seconds = 0, rdm_gemm_ms = 0;
     double rdm_stream_bytes = 0;                  // bytes of the launches of the HBM-bound streaming kernel alone
     double t_plan = 0, t_davidson = 0, t_split = 0, t_grow = 0, t_matvec = 0;   // phase seconds of the last sweep

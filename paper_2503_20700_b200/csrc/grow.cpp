@@ -208,7 +208,7 @@ static void rotate_batch(Block& X, const Dot& dot, const SiteTensor& tensor, Blo
     std::vector<OpPlan> plans(list.size());
     std::string err;
     int err_code = 0;
-#pragma omp parallel for schedule(dynamic, 4)
+#pragma omp parallel for schedule(dynamic, 4) if (list.size() > 32)
     for (long j = 0; j < (long)list.size(); ++j) {
         try {
             plan_op(X, dot, tensor, nb, list[j], cap, plans[j]);
@@ -247,7 +247,7 @@ enum OpWhat : int { W_H, W_CRE, W_ST, W_A, W_B, W_COPY };
 struct OpSpec { Label label; int what; };
 static std::vector<NewOp> make_ops(const std::vector<OpSpec>& specs, const Gen& gen) {
     std::vector<NewOp> out(specs.size());
-#pragma omp parallel for schedule(dynamic, 16)
+#pragma omp parallel for schedule(dynamic, 16) if (specs.size() > 256)
     for (long j = 0; j < (long)specs.size(); ++j) {
         const Label& l = specs[j].label;
         NewOp& o = out[j];

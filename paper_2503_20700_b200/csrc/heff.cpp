@@ -75,7 +75,7 @@ static std::vector<NTerm> heff_terms(const Ham& ham, Block& LB, Block& RB, const
             for (int S : A)
                 for (Term t : gen.B(P, S)) { t.f.push_back(yf(L2(K_Q, P, S), false)); T.push_back(t); }
     std::vector<NTerm> out(T.size());                          // 16 x 16 dot-matrix products per term: host threads
-#pragma omp parallel for schedule(static, 64)
+#pragma omp parallel for schedule(static, 64) if (T.size() > 1024)
     for (long j = 0; j < (long)T.size(); ++j) out[j] = normalise(T[j], "LdR", dot);
     return out;
 }
@@ -222,7 +222,7 @@ static void build_maps_device(HeffPlan& p, const std::vector<NTerm>& terms, Bloc
         // the tiles of one output block closer together in time, which helps the L2 hit rate of their shared panels
         const int64_t target = (int64_t)sms * 3 * 64;
         if (base_tiles > 0) S = (int)std::min<int64_t>(16, std::max<int64_t>(1, (target + base_tiles - 1) / base_tiles));
-        if (eng.opt.split_k > 0) S = std::min(16, eng.opt.split_k);
+        if (eng.opt.split_k > 0) S = std::min(64, eng.opt.split_k);
     }
     p.split = S;
     if (S > 1) p.ypart.alloc((size_t)(S - 1) * (size_t)std::max<int64_t>(p.nnz, 1));

@@ -515,7 +515,7 @@ void move_centre_right(const SiteTensor& psi, const Basis& bl, const Basis& br, 
     // sector SVDs concurrently: a few host threads, each with its own stream and cuSOLVER handle (psi is complete: the
     // previous step ended synchronised)
     cuda_check(cudaStreamSynchronize(st), "rdm centre move");
-    const int nthreads = 4;
+    const int nthreads = eng.host_threads;
     eng.ensure_svd_pool(nthreads);
     std::string err;
     int64_t nlaunch = 0;
@@ -584,7 +584,7 @@ void move_centre_left(const SiteTensor& psi, const Basis& bl, const Basis& br, c
     std::vector<DevVec<double>> lms(bl.size());
     GemmBatch gb;
     cuda_check(cudaStreamSynchronize(st), "rdm centre move");
-    const int nthreads = 4;
+    const int nthreads = eng.host_threads;
     eng.ensure_svd_pool(nthreads);
     std::string err;
     int64_t nlaunch = 0;

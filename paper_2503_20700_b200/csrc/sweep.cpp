@@ -325,7 +325,7 @@ void split_theta(MPS& mps, int i, const HeffPlan& p, const double* theta, int D,
     // The sector SVDs are independent and individually too small to fill the device: a few host threads run them
     // concurrently, each on its own stream and cuSOLVER handle (theta is complete: Davidson ended synchronised).
     // Largest sectors first.
-    const int nthreads = 4;
+    const int nthreads = eng.host_threads;
     eng.ensure_svd_pool(nthreads);
     std::vector<int> by_size(order.size());
     for (size_t j = 0; j < order.size(); ++j) by_size[j] = (int)j;
@@ -497,7 +497,6 @@ void Engine::plan_env_policy(int D) {
         int s = 1;
         while (s < k && total / s > host_budget) ++s;
         if ((s + 1) * bmax > budget) throw Error(-3, "environment stack: one segment between host checkpoints exceeds the device budget");
-        while (s + 1 < k && (s + 2) * bmax <= 0.5 * budget) ++s;      // fewer, larger segments: fewer host round trips
         env_stride = s; env_spill = true;
         return;
     }

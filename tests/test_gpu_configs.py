@@ -61,7 +61,11 @@ def _compare(lib, cfg, D, bonds, seed):
 
 
 def test_config2_coronene_D512_heff_vs_oracle(lib):
-    _compare(lib, make_config(2), 512, list(range(0, 23, 2)), seed=2001)      # every second two-site bond, ends included
+    _compare(lib, make_config(2), 512, [0, 4, 8, 10, 11, 12, 16, 22], seed=2001)   # full D: ends, around the N/C switch, between
+
+
+def test_config2_coronene_every_bond_heff_vs_oracle(lib):
+    _compare(lib, make_config(2), 160, list(range(0, 23)), seed=2003)             # EVERY two-site bond
 
 
 def test_config3_fes_D1024_midbond_heff_vs_oracle(lib):
