@@ -26,8 +26,10 @@
 #include <algorithm>
 #include <chrono>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 
+#include <cuda_profiler_api.h>
 #include <omp.h>
 
 #include "core.hpp"
@@ -189,6 +191,10 @@ struct Evaluator {
         eng.rdm_flops += p1.flops + p2.flops + pe.flops;
         run_once(p1, eng);
         run_once(p2, eng);
+        // DMRG_B200_PROFILE_RDM=1 (diagnostics): open the profiler range around the accumulation launches only, so that
+        // `ncu --profile-from-start off` lists exactly the E = Stack M^T kernels of the pass
+        static const bool prof = [] { const char* g = std::getenv("DMRG_B200_PROFILE_RDM"); return g && g[0] == '1'; }();
+        if (prof) cudaProfilerStart();
         if (!dots.empty()) {
             cudaEventRecord(e0, st);
             for (const DotsCall& d : dots) {
@@ -210,6 +216,7 @@ struct Evaluator {
             run(lr, eng);
         }
         cuda_check(cudaStreamSynchronize(st), "rdm accumulation");
+        if (prof) cudaProfilerStop();
         float ms = 0.f;
         if (!dots.empty()) { cudaEventElapsedTime(&ms, e0, e1); eng.rdm_stream_ms += ms; }
         if (gem) { cudaEventElapsedTime(&ms, e2, e3); eng.rdm_gemm_ms += ms; }
