@@ -164,7 +164,7 @@ def test_dbss_sweep_matches_oracle(lib, k, n, s2, eps, dmin, dmax):
     try:
         lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, s2)
         kept = set()
-        for _ in range(3):
+        for _ in range(2):
             g, o = lib.dmrg_sweep(ctx, dmax, k), eng.sweep(dmax)
             assert abs(g["energy_last"] - o["energy_last"]) <= TOL_E
             for rg, ro in zip(g["bonds"], o["bonds"]):
@@ -176,7 +176,7 @@ def test_dbss_sweep_matches_oracle(lib, k, n, s2, eps, dmin, dmax):
         lib.dmrg_destroy(ctx)
 
 
-@pytest.mark.parametrize("k,n,s2,D", [(6, 6, 0, 12), (8, 9, 1, 24)])
+@pytest.mark.parametrize("k,n,s2,D", [(6, 6, 0, 12), (7, 8, 2, 16)])
 def test_lanczos_sweep_matches_oracle(lib, k, n, s2, D):
     """Lanczos as the local eigensolver (reading S33): converged to 1e-10 it reaches the same eigenpairs as
     the oracle's Lanczos (and Davidson), so the whole sweep agrees."""
@@ -200,16 +200,16 @@ def test_lanczos_sweep_matches_oracle(lib, k, n, s2, D):
 def test_solve_stops_by_eps_sweep_like_the_oracle(lib):
     """dmrg_solve: the eps_sweep rule of PAPER.md:179 (reading S34) stops after the same number of sweeps as the oracle's
     SweepEngine.solve, at the same energy."""
-    k, n, s2, D = 8, 8, 0, 20
+    k, n, s2, D = 5, 5, 1, 8
     h, eri = random_dense(k, 640)
     mps = random_mps(k, n, s2, D, seed=12, gauge="R")
     ctx = lib.dmrg_create(k, n, s2, h, eri, davidson_tol=1e-10)
     try:
         lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, s2)
-        r = lib.dmrg_solve(ctx, D, k, 1e-6, 15)
+        r = lib.dmrg_solve(ctx, D, k, 1e-5, 15)
     finally:
         lib.dmrg_destroy(ctx)
-    out = odmrg.SweepEngine(h, eri, mps, davidson_tol=1e-10).solve(D, 1e-6, 15)
+    out = odmrg.SweepEngine(h, eri, mps, davidson_tol=1e-10).solve(D, 1e-5, 15)
     assert r["status"] == 0 and r["n_sweeps"] == len(out) and 3 <= len(out) < 15
     assert np.abs(r["energies"] - np.array([o["energy_last"] for o in out])).max() <= TOL_E
     assert abs(r["last"]["energy_last"] - out[-1]["energy_last"]) <= TOL_E
