@@ -130,6 +130,7 @@ int dmrg_create(dmrg_ctx** out, int k, int n_elec, int two_sz, const double* h, 
         eng.ham.h.assign(h, h + (size_t)k * k);
         eng.ham.eri.assign(eri, eri + (size_t)k * k * k * k);
         eng.host_threads = std::max(1, std::min(8, omp_get_num_procs()));
+        if (const char* g = std::getenv("DMRG_B200_HOST_THREADS")) eng.host_threads = std::max(1, std::min(64, std::atoi(g)));   // diagnostics: A/B of the host team size
         omp_set_num_threads(eng.host_threads);
         eng.svd = svd_create(eng.stream, eng.opt.svd_qr == 0);
         eng.red_scratch.alloc((size_t)multi_dot_scratch());

@@ -1,8 +1,10 @@
 // Device-resident block operators: storage, launch-descriptor plumbing, linear combinations, blocking (grow).
 #include <algorithm>
 #include <cassert>
+#include <chrono>
 #include <cmath>
 #include <cstdio>
+#include <cstring>
 #include <mutex>
 
 #include "core.hpp"
@@ -39,6 +41,20 @@ void dev_free(void* p) {
     }
     cudaFree(p);
 }
+
+void* PinnedBuf::get(size_t n) {
+    if (n <= bytes) return p;
+    if (p) cudaFreeHost(p);
+    p = nullptr;
+    bytes = n + n / 2 + 4096;
+    if (cudaHostAlloc(&p, bytes, cudaHostAllocDefault) != cudaSuccess) {
+        cudaGetLastError();
+        p = nullptr; bytes = 0;
+        throw Error(-3, "pinned host memory exhausted (descriptor staging)");
+    }
+    return p;
+}
+PinnedBuf::~PinnedBuf() { if (p) cudaFreeHost(p); }
 
 int find_sector(const Basis& b, int n, int s) {
     int lo = 0, hi = (int)b.size() - 1;
@@ -92,22 +108,30 @@ void finalize(GemmBatch& b, GemmLaunch& out, Engine& eng) {
     // (K <= 0 or alpha == 0) are dropped.  Equal alphas adjacent let the bulk-copy kernel keep its accumulators in
     // units of the current alpha and rescale them only when alpha changes (no per-fragment multiply in the main loop).
     // Counting sort of the segments by task (stable), then one small sort per task - tasks in parallel on the host.
-    std::vector<int> off((size_t)nt + 1, 0);
+    FinalizeScratch& fs = eng.fin;
+    std::vector<int>& off = fs.off;
+    off.assign((size_t)nt + 1, 0);
     for (size_t j = 0; j < ns; ++j) {
         const Seg& sg = b.segs[j];
         if (!(sg.flags & SEG_IDENT_B) && (sg.K <= 0 || sg.alpha == 0.0)) continue;
         off[(size_t)b.seg_task[j] + 1]++;
     }
     for (int t = 0; t < nt; ++t) off[t + 1] += off[t];
-    std::vector<int> idx((size_t)off[nt]), fill(off.begin(), off.end() - 1);
+    std::vector<int>& idx = fs.idx;
+    std::vector<int>& fill = fs.fill;
+    idx.resize((size_t)off[nt]);
+    fill.assign(off.begin(), off.end() - 1);
     for (size_t j = 0; j < ns; ++j) {
         const Seg& sg = b.segs[j];
         if (!(sg.flags & SEG_IDENT_B) && (sg.K <= 0 || sg.alpha == 0.0)) continue;
         idx[(size_t)fill[b.seg_task[j]]++] = (int)j;
     }
-    std::vector<Seg> sorted((size_t)off[nt]);
-    std::vector<double> weight(nt, 0.0);
-    std::vector<int> ntile((size_t)nt + 1, 0);
+    const size_t nsorted = (size_t)off[nt];
+    Seg* sorted = (Seg*)fs.segs.get(std::max<size_t>(nsorted, 1) * sizeof(Seg));
+    std::vector<double>& weight = fs.weight;
+    std::vector<int>& ntile = fs.ntile;
+    weight.assign(nt, 0.0);
+    ntile.assign((size_t)nt + 1, 0);
     int aligned_i = 1;
 #pragma omp parallel for schedule(static, 256) reduction(&& : aligned_i) if (nt > 4096)
     for (int t = 0; t < nt; ++t) {
@@ -153,8 +177,10 @@ void finalize(GemmBatch& b, GemmLaunch& out, Engine& eng) {
     // launch on short tiles
     for (int t = 0; t < nt; ++t) ntile[(size_t)t + 1] += ntile[t];
     const size_t ntl = (size_t)ntile[nt];
-    std::vector<Tile> raw(ntl);
-    std::vector<double> tw(ntl);
+    std::vector<Tile>& raw = fs.raw;
+    std::vector<double>& tw = fs.tw;
+    raw.resize(ntl);
+    tw.resize(ntl);
 #pragma omp parallel for schedule(static, 256) if (nt > 4096)
     for (int t = 0; t < nt; ++t) {
         const Task& tk = b.tasks[t];
@@ -186,8 +212,10 @@ void finalize(GemmBatch& b, GemmLaunch& out, Engine& eng) {
     // stable counting sort by weight, heaviest first, on 1/16-octave buckets (the order only balances the load: results do
     // not depend on it, every tile is owned by one CTA and its summation order is the segment order)
     constexpr int NB = 1024;
-    std::vector<int> bucket(ntl);
-    std::vector<size_t> hist(NB + 1, 0);
+    std::vector<int>& bucket = fs.bucket;
+    std::vector<size_t>& hist = fs.hist;
+    bucket.resize(ntl);
+    hist.assign(NB + 1, 0);
     for (size_t j = 0; j < ntl; ++j) {
         int q = (int)(std::log2(std::max(tw[j], 1.0)) * 16.0);
         q = NB - 1 - std::min(NB - 1, std::max(0, q));          // heavy tiles -> low bucket
@@ -195,13 +223,15 @@ void finalize(GemmBatch& b, GemmLaunch& out, Engine& eng) {
         hist[(size_t)q + 1]++;
     }
     for (int q = 0; q < NB; ++q) hist[(size_t)q + 1] += hist[q];
-    std::vector<Tile> tiles(ntl);
+    Tile* tiles = (Tile*)fs.tiles.get(std::max<size_t>(ntl, 1) * sizeof(Tile));
     for (size_t j = 0; j < ntl; ++j) tiles[hist[bucket[j]]++] = raw[j];
-    out.tasks.upload(b.tasks, eng.stream);
-    out.segs.upload(sorted, eng.stream);
-    out.tiles.upload(tiles, eng.stream);
+    Task* ptasks = (Task*)fs.tasks.get(std::max<size_t>((size_t)nt, 1) * sizeof(Task));
+    std::memcpy(ptasks, b.tasks.data(), (size_t)nt * sizeof(Task));
+    out.tasks.upload_raw(ptasks, (size_t)nt, eng.stream);
+    out.segs.upload_raw(sorted, nsorted, eng.stream);
+    out.tiles.upload_raw(tiles, ntl, eng.stream);
     if (!out.counter.p) out.counter.alloc(1);
-    out.ntiles = (int)tiles.size();
+    out.ntiles = (int)ntl;
     out.flops = b.flops;
     cuda_check(cudaStreamSynchronize(eng.stream), "descriptor upload");   // host vectors die after this call
 }
@@ -232,7 +262,11 @@ void run(const GemmLaunch& l, Engine& eng, cudaStream_t st) {
 void run_once(GemmBatch& b, Engine& eng) {
     if (b.tasks.empty()) return;
     GemmLaunch l;
+    const auto t0 = std::chrono::steady_clock::now();
     finalize(b, l, eng);
+    if (eng.trace)
+        std::fprintf(stderr, "[dmrg trace] finalize tasks=%zu segs=%zu host=%.4f s\n", b.tasks.size(), b.segs.size(),
+                     std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count());
     run(l, eng);
     cuda_check(cudaStreamSynchronize(eng.stream), "grouped GEMM");
     b = GemmBatch();

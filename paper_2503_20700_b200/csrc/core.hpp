@@ -40,6 +40,10 @@ struct DevVec {
     ~DevVec() { release(); }
     void release() { if (p) dev_free(p); p = nullptr; n = 0; }
     void alloc(size_t n_) { release(); n = n_; if (n) p = (T*)dev_alloc(n * sizeof(T)); }
+    void upload_raw(const T* src, size_t count, cudaStream_t st) {
+        if (count > n) alloc(count);
+        if (count) cuda_check(cudaMemcpyAsync(p, src, count * sizeof(T), cudaMemcpyHostToDevice, st), "upload");
+    }
     void upload(const std::vector<T>& v, cudaStream_t st) {
         if (v.size() > n) alloc(v.size());
         if (!v.empty()) cuda_check(cudaMemcpyAsync(p, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice, st), "upload");
@@ -87,6 +91,24 @@ struct GemmLaunch {                               // device-resident descriptors
     int ntiles = 0;
     bool aligned = false;                         // every GEMM operand 16-byte aligned, even ld: bulk-copy kernel
     double flops = 0.0;
+};
+// Growable pinned host buffer: descriptor tables are written straight into it and uploaded by DMA (a pageable source is
+// staged by the driver at a fraction of the rate, and fresh 100 MB vectors page-fault on every call).
+struct PinnedBuf {
+    void* p = nullptr;
+    size_t bytes = 0;
+    void* get(size_t n);
+    PinnedBuf() {}
+    PinnedBuf(const PinnedBuf&) = delete;
+    PinnedBuf& operator=(const PinnedBuf&) = delete;
+    ~PinnedBuf();
+};
+struct FinalizeScratch {                          // reused by every finalize() of a context (capacity is kept)
+    PinnedBuf segs, tiles, tasks;
+    std::vector<int> off, idx, fill, ntile, bucket;
+    std::vector<double> weight, tw;
+    std::vector<Tile> raw;
+    std::vector<size_t> hist;
 };
 struct Engine;
 void finalize(GemmBatch& b, GemmLaunch& out, Engine& eng);   // sort segs by task, build tiles, upload
@@ -257,6 +279,7 @@ struct Engine {
     std::vector<SvdWork*> svd_pool;               // extra cuSOLVER handles on their own streams: sector SVDs run concurrently
     std::vector<cudaStream_t> svd_streams;
     void ensure_svd_pool(int n);
+    FinalizeScratch fin;
     int host_threads = 1;                         // size of the one OpenMP team every host-parallel region uses (a changing
                                                   // team size makes libgomp rebuild its thread pool at every region)
     double rdm_seconds = 0, rdm_bytes = 0, rdm_flops = 0, rdm_host_seconds = 0, rdm_grow_seconds = 0, rdm_gemm_ms = 0;

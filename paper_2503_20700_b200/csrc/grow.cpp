@@ -6,6 +6,8 @@
 // both phases are launches of the grouped FP64 GEMM kernel over all new operators of a chunk.
 #include <algorithm>
 #include <cassert>
+#include <chrono>
+#include <cstdio>
 
 #include "core.hpp"
 
@@ -180,20 +182,40 @@ static void plan_op(Block& X, const Dot& dot, const SiteTensor& tensor, Block& n
     }
 }
 
-// append the plan of one operator to the launch-wide batches: task indices shifted, workspace offsets turned into
-// addresses at `base`
-static void merge(GemmBatch& p1, GemmBatch& p2, const OpPlan& pl, double* base) {
-    const int t1 = (int)p1.tasks.size(), t2 = (int)p2.tasks.size();
-    const size_t s2 = p2.segs.size();
-    for (Task t : pl.p1.tasks) { t.C = base + (t.C - (double*)nullptr); p1.tasks.push_back(t); }
-    p1.segs.insert(p1.segs.end(), pl.p1.segs.begin(), pl.p1.segs.end());
-    for (int t : pl.p1.seg_task) p1.seg_task.push_back(t1 + t);
-    p1.flops += pl.p1.flops;
-    p2.tasks.insert(p2.tasks.end(), pl.p2.tasks.begin(), pl.p2.tasks.end());
-    p2.segs.insert(p2.segs.end(), pl.p2.segs.begin(), pl.p2.segs.end());
-    for (int j : pl.tsegs) p2.segs[s2 + j].B = base + (p2.segs[s2 + j].B - (const double*)nullptr);
-    for (int t : pl.p2.seg_task) p2.seg_task.push_back(t2 + t);
-    p2.flops += pl.p2.flops;
+// append the plans [j0, j1) to the launch-wide batches in list order: task indices shifted, workspace offsets turned into
+// addresses (plan j starts at base + toff[j]).  Sizes are prefix-summed first, then the copies run on the host threads.
+static void merge_range(GemmBatch& p1, GemmBatch& p2, const std::vector<OpPlan>& plans, size_t j0, size_t j1,
+                        const std::vector<int64_t>& toff, double* base) {
+    const size_t n = j1 - j0;
+    std::vector<size_t> t1(n + 1, 0), s1(n + 1, 0), t2(n + 1, 0), s2(n + 1, 0);
+    for (size_t j = 0; j < n; ++j) {
+        const OpPlan& pl = plans[j0 + j];
+        t1[j + 1] = t1[j] + pl.p1.tasks.size(); s1[j + 1] = s1[j] + pl.p1.segs.size();
+        t2[j + 1] = t2[j] + pl.p2.tasks.size(); s2[j + 1] = s2[j] + pl.p2.segs.size();
+        p1.flops += pl.p1.flops; p2.flops += pl.p2.flops;
+    }
+    p1.tasks.resize(t1[n]); p1.segs.resize(s1[n]); p1.seg_task.resize(s1[n]);
+    p2.tasks.resize(t2[n]); p2.segs.resize(s2[n]); p2.seg_task.resize(s2[n]);
+#pragma omp parallel for schedule(dynamic, 8) if (n > 32)
+    for (long j = 0; j < (long)n; ++j) {
+        const OpPlan& pl = plans[j0 + j];
+        double* tb = base + toff[j0 + j];
+        for (size_t q = 0; q < pl.p1.tasks.size(); ++q) {
+            Task t = pl.p1.tasks[q];
+            t.C = tb + (t.C - (double*)nullptr);
+            p1.tasks[t1[j] + q] = t;
+        }
+        for (size_t q = 0; q < pl.p1.segs.size(); ++q) {
+            p1.segs[s1[j] + q] = pl.p1.segs[q];
+            p1.seg_task[s1[j] + q] = (int)t1[j] + pl.p1.seg_task[q];
+        }
+        for (size_t q = 0; q < pl.p2.tasks.size(); ++q) p2.tasks[t2[j] + q] = pl.p2.tasks[q];
+        for (size_t q = 0; q < pl.p2.segs.size(); ++q) {
+            p2.segs[s2[j] + q] = pl.p2.segs[q];
+            p2.seg_task[s2[j] + q] = (int)t2[j] + pl.p2.seg_task[q];
+        }
+        for (int q : pl.tsegs) { Seg& sg = p2.segs[s2[j] + q]; sg.B = tb + (sg.B - (const double*)nullptr); }
+    }
 }
 
 static void rotate_batch(Block& X, const Dot& dot, const SiteTensor& tensor, Block& nb, const std::vector<NewOp>& list,
@@ -208,6 +230,7 @@ static void rotate_batch(Block& X, const Dot& dot, const SiteTensor& tensor, Blo
     std::vector<OpPlan> plans(list.size());
     std::string err;
     int err_code = 0;
+    const auto tp0 = std::chrono::steady_clock::now();
 #pragma omp parallel for schedule(dynamic, 4) if (list.size() > 32)
     for (long j = 0; j < (long)list.size(); ++j) {
         try {
@@ -221,25 +244,45 @@ static void rotate_batch(Block& X, const Dot& dot, const SiteTensor& tensor, Blo
         }
     }
     if (err_code) { if (err_code == -3) throw Error(-3, err); throw std::logic_error(err); }
+    const auto tp1 = std::chrono::steady_clock::now();
     int64_t total = 0;
     for (const OpPlan& pl : plans) total += pl.used;
     DevVec<double> tmp;
     tmp.alloc((size_t)std::max<int64_t>(2, std::min(total, cap)));
     GemmBatch p1, p2;
     int64_t used = 0;
+    double t_run = 0.0;
     auto flush = [&]() {
+        const auto a = std::chrono::steady_clock::now();
         run_once(p1, eng);
         run_once(p2, eng);
+        t_run += std::chrono::duration<double>(std::chrono::steady_clock::now() - a).count();
         used = 0;
     };
-    for (OpPlan& pl : plans) {
-        if (used + pl.used > cap) flush();
-        merge(p1, p2, pl, tmp.p + used);
-        used += pl.used;
-        pl = OpPlan();
-        if (used > cap / 2 && total > cap) flush();
+    // flush groups: consecutive plans whose workspace fits (one group when everything fits)
+    std::vector<int64_t> toff(plans.size(), 0);
+    size_t j = 0;
+    while (j < plans.size()) {
+        const size_t g0 = j;
+        used = 0;
+        while (j < plans.size()) {
+            if (used + plans[j].used > cap) break;            // does not fit: the group closes before plan j
+            toff[j] = used;
+            used += plans[j].used;
+            ++j;
+            if (total > cap && used > cap / 2) break;         // several flushes: close at half the workspace
+        }
+        if (j == g0) throw Error(-3, "renormalisation workspace too small");
+        merge_range(p1, p2, plans, g0, j, toff, tmp.p);
+        for (size_t q = g0; q < j; ++q) plans[q] = OpPlan();
+        flush();
     }
-    flush();
+    if (eng.trace) {
+        const double all = std::chrono::duration<double>(std::chrono::steady_clock::now() - tp0).count();
+        const double plan = std::chrono::duration<double>(tp1 - tp0).count();
+        std::fprintf(stderr, "[dmrg trace] rotate_batch ops=%zu plan=%.4f merge=%.4f finalize+run=%.4f s\n", list.size(), plan,
+                     all - plan - t_run, t_run);
+    }
 }
 
 // symbolic expressions of a list of new operators, generated by the host threads (the generator is read-only)
