@@ -53,30 +53,62 @@ static std::vector<NTerm> heff_terms(const Ham& ham, Block& LB, Block& RB, const
     std::vector<int> A = X->inside();
     A.insert(A.end(), dot.so.begin(), dot.so.end());
     std::sort(A.begin(), A.end());
-    Expr T = gen.H(), G;
+    // The term list in its fixed order: H_A, H_Y, G, G^+, B Q with G = a+_P^A S_P^Y, a+_P^Y S_P^A, A_PQ^A P_PQ^Y.  Each
+    // entry of `jobs` yields a few terms; the host threads generate and normalise them (16 x 16 dot-matrix products per
+    // term), the results are concatenated in job order, so the list does not depend on the number of threads.
+    struct Job { int kind, a, b; };                            // 0: H_A, 1: H_Y, 2: cre(a) St_a^Y, 3: C_a^Y S(a), 4: A(a,b) Pt^Y, 5: B(a,b) Q^Y
+    std::vector<Job> jobs;
+    jobs.push_back({0, 0, 0});
     if (!Yin.empty()) {
-        { Term t; t.f.push_back(yf(L0(K_H), false)); T.push_back(t); }
-        for (int P : A)                                        // a+_P^A S_P^Y
-            for (Term t : gen.cre(P)) { t.f.push_back(yf(L1(K_St, P), true)); G.push_back(t); }
-        for (int P : Yin)                                      // a+_P^Y S_P^A
-            for (const Term& s : gen.S(P)) {
-                Term t; t.coef = s.coef; t.f.push_back(yf(L1(K_C, P), false));
-                t.f.insert(t.f.end(), s.f.begin(), s.f.end());
-                G.push_back(t);
-            }
-        for (size_t a = 0; a < A.size(); ++a)                  // A_PQ^A P_PQ^Y
-            for (size_t b = a + 1; b < A.size(); ++b)
-                for (Term t : gen.A(A[a], A[b])) { t.f.push_back(yf(L2(K_Pt, A[a], A[b]), true)); G.push_back(t); }
+        jobs.push_back({1, 0, 0});
+        for (int P : A) jobs.push_back({2, P, 0});
+        for (int P : Yin) jobs.push_back({3, P, 0});
+        for (size_t a = 0; a < A.size(); ++a)
+            for (size_t b = a + 1; b < A.size(); ++b) jobs.push_back({4, A[a], A[b]});
+        for (int P : A)
+            for (int S : A) jobs.push_back({5, P, S});
     }
-    for (const Term& t : G) T.push_back(t);
-    for (const Term& t : G) T.push_back(adjoint(t));
-    if (!Yin.empty())
-        for (int P : A)                                        // B_PS^A Q_PS^Y
-            for (int S : A)
-                for (Term t : gen.B(P, S)) { t.f.push_back(yf(L2(K_Q, P, S), false)); T.push_back(t); }
-    std::vector<NTerm> out(T.size());                          // 16 x 16 dot-matrix products per term: host threads
-#pragma omp parallel for schedule(static, 64) if (T.size() > 1024)
-    for (long j = 0; j < (long)T.size(); ++j) out[j] = normalise(T[j], "LdR", dot);
+    std::vector<std::vector<NTerm>> fwd(jobs.size()), adj(jobs.size());
+    std::string err;
+#pragma omp parallel for schedule(dynamic, 16) if (jobs.size() > 256)
+    for (long j = 0; j < (long)jobs.size(); ++j) {
+        try {
+            const Job& jb = jobs[j];
+            Expr e;
+            bool hc = false;
+            switch (jb.kind) {
+                case 0: e = gen.H(); break;
+                case 1: { Term t; t.f.push_back(yf(L0(K_H), false)); e.push_back(t); break; }
+                case 2: for (Term t : gen.cre(jb.a)) { t.f.push_back(yf(L1(K_St, jb.a), true)); e.push_back(t); } hc = true; break;
+                case 3:
+                    for (const Term& sT : gen.S(jb.a)) {
+                        Term t; t.coef = sT.coef; t.f.push_back(yf(L1(K_C, jb.a), false));
+                        t.f.insert(t.f.end(), sT.f.begin(), sT.f.end());
+                        e.push_back(t);
+                    }
+                    hc = true; break;
+                case 4: for (Term t : gen.A(jb.a, jb.b)) { t.f.push_back(yf(L2(K_Pt, jb.a, jb.b), true)); e.push_back(t); } hc = true; break;
+                default: for (Term t : gen.B(jb.a, jb.b)) { t.f.push_back(yf(L2(K_Q, jb.a, jb.b), false)); e.push_back(t); }
+            }
+            for (const Term& t : e) {
+                fwd[j].push_back(normalise(t, "LdR", dot));
+                if (hc) adj[j].push_back(normalise(adjoint(t), "LdR", dot));
+            }
+        } catch (const std::exception& ex) {
+#pragma omp critical
+            err = ex.what();
+        }
+    }
+    if (!err.empty()) throw std::logic_error(err);
+    std::vector<NTerm> out;
+    auto append = [&](int kind, std::vector<std::vector<NTerm>>& src) {
+        for (size_t j = 0; j < jobs.size(); ++j)
+            if (jobs[j].kind == kind) for (NTerm& t : src[j]) out.push_back(std::move(t));
+    };
+    append(0, fwd); append(1, fwd);
+    for (int kind : {2, 3, 4}) append(kind, fwd);
+    for (int kind : {2, 3, 4}) append(kind, adj);
+    append(5, fwd);
     return out;
 }
 
