@@ -64,6 +64,7 @@ def parse_args():
     ap.add_argument("--max-iter", type=int, default=12, help="Davidson iterations per bond of --big sweeps")
     ap.add_argument("--host-spill", type=int, default=1)
     ap.add_argument("--env-stride", type=int, default=0)
+    ap.add_argument("--env-stride2", type=int, default=0)
     ap.add_argument("--hbm-budget-gb", type=float, default=0.0)
     ap.add_argument("--host-budget-gb", type=float, default=0.0)
     ap.add_argument("--cpu-baseline", type=int, default=1)
@@ -331,7 +332,8 @@ def run_big(args):
     import paper_2503_20700_b200 as P
     torch.cuda.set_device(0)
     peaks = measured_peaks()
-    opts = dict(davidson_max_iter=args.max_iter, host_spill=args.host_spill, env_stride=args.env_stride)
+    opts = dict(davidson_max_iter=args.max_iter, host_spill=args.host_spill, env_stride=args.env_stride,
+                env_stride2=args.env_stride2)
     if args.hbm_budget_gb > 0:
         opts["hbm_budget_bytes"] = int(args.hbm_budget_gb * (1 << 30))
     if args.host_budget_gb > 0:

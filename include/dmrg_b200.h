@@ -61,7 +61,8 @@ typedef struct dmrg_options {
                                      third-smallest site < kh are evaluated there with the two-index operators on the left,
                                      the others at their second-smallest site with them on the right); 0 and k give the two
                                      one-sided evaluation orders.  Results do not depend on it (tested); memory does.       */
-    int32_t reserved0;
+    int32_t env_stride2;          /* default 0 = automatic: second checkpoint level inside a segment - of the blocks recomputed
+                                     from a checkpoint only every env_stride2-th and the sub-segment in use stay resident      */
 } dmrg_options;
 
 /* Neutral MPS exchange format (host memory, caller-owned, flat arrays).
@@ -170,7 +171,7 @@ typedef struct dmrg_sweep_stats_t {
     double seconds_maps, seconds_davidson, seconds_matvec, seconds_split, seconds_renormalise;
     double bytes_spilled, bytes_restored;
     int64_t peak_device_bytes, host_pool_bytes, est_stack_bytes, est_max_block_bytes;
-    int32_t env_stride, host_spill;
+    int32_t env_stride, host_spill, env_stride2, reserved;
 } dmrg_sweep_stats_t;
 int dmrg_sweep_stats(dmrg_ctx* ctx, dmrg_sweep_stats_t* out);
 

@@ -29,7 +29,7 @@ class dmrg_options(C.Structure):
                 ("hbm_budget_bytes", C.c_int64), ("host_budget_bytes", C.c_int64), ("host_spill", C.c_int32),
                 ("env_stride", C.c_int32), ("dbss_eps", C.c_double), ("dbss_dmin", C.c_int32), ("split_k", C.c_int32),
                 ("svd_qr", C.c_int32), ("host_maps", C.c_int32), ("generic_gemm", C.c_int32), ("eigensolver", C.c_int32),
-                ("rdm_split", C.c_int32), ("reserved0", C.c_int32)]
+                ("rdm_split", C.c_int32), ("env_stride2", C.c_int32)]
 
 
 class dmrg_mps_blob(C.Structure):
@@ -215,7 +215,7 @@ class dmrg_sweep_stats_t(C.Structure):
                                           "seconds_spill_wait", "seconds_maps", "seconds_davidson", "seconds_matvec",
                                           "seconds_split", "seconds_renormalise", "bytes_spilled", "bytes_restored")] + \
                [(n, C.c_int64) for n in ("peak_device_bytes", "host_pool_bytes", "est_stack_bytes", "est_max_block_bytes")] + \
-               [("env_stride", C.c_int32), ("host_spill", C.c_int32)]
+               [("env_stride", C.c_int32), ("host_spill", C.c_int32), ("env_stride2", C.c_int32), ("reserved", C.c_int32)]
 
 
 def dmrg_sweep_stats(ctx):

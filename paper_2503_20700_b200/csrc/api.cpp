@@ -79,7 +79,7 @@ void dmrg_default_options(dmrg_options* o) {
     o->workspace_bytes = 0;
     o->hbm_budget_bytes = 0; o->host_budget_bytes = 0; o->host_spill = 0; o->env_stride = 0;
     o->dbss_eps = 0.0; o->dbss_dmin = 0; o->split_k = 0; o->svd_qr = 0; o->host_maps = 0; o->generic_gemm = 0;
-    o->eigensolver = 0; o->rdm_split = -1; o->reserved0 = 0;
+    o->eigensolver = 0; o->rdm_split = -1; o->env_stride2 = 0;
 }
 
 int dmrg_create(dmrg_ctx** out, int k, int n_elec, int two_sz, const double* h, const double* eri,
@@ -111,7 +111,7 @@ int dmrg_create(dmrg_ctx** out, int k, int n_elec, int two_sz, const double* h, 
             eng.opt.dbss_eps = opt->dbss_eps; eng.opt.dbss_dmin = opt->dbss_dmin;
             eng.opt.split_k = opt->split_k; eng.opt.svd_qr = opt->svd_qr;
             eng.host_maps = opt->host_maps != 0; eng.force_generic_gemm = opt->generic_gemm != 0;
-            eng.opt.eigensolver = opt->eigensolver; eng.opt.rdm_split = opt->rdm_split;
+            eng.opt.eigensolver = opt->eigensolver; eng.opt.rdm_split = opt->rdm_split; eng.opt.env_stride2 = opt->env_stride2;
         }
         if (eng.opt.davidson_max_subspace < 2 || eng.opt.davidson_max_subspace > COMBINE_MAX ||
             eng.opt.davidson_max_iter < 1 || !(eng.opt.davidson_tol > 0) || eng.opt.env_stride < 0 ||
@@ -431,7 +431,7 @@ int dmrg_sweep_stats(dmrg_ctx* ctx, dmrg_sweep_stats_t* out) {
     out->bytes_spilled = eng.spill_bytes; out->bytes_restored = eng.restore_bytes;
     out->peak_device_bytes = eng.env_peak_bytes; out->host_pool_bytes = eng.host_pool.bytes;
     out->est_stack_bytes = eng.env_est_total; out->est_max_block_bytes = eng.env_est_max;
-    out->env_stride = eng.env_stride; out->host_spill = eng.env_spill ? 1 : 0;
+    out->env_stride = eng.env_stride; out->host_spill = eng.env_spill ? 1 : 0; out->env_stride2 = eng.env_stride2; out->reserved = 0;
     return DMRG_OK;
     API_END
 }

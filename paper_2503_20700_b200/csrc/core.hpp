@@ -247,6 +247,7 @@ struct Options {
     int64_t host_budget_bytes = 0;                // pinned host bytes for spilled checkpoints (0 = automatic: 64 GiB)
     int host_spill = 0;                           // 1: environment checkpoints may live in pinned host memory
     int env_stride = 0;                           // checkpoint spacing of the environment stack (0 = automatic, 1 = keep all)
+    int env_stride2 = 0;                          // second checkpoint level inside a segment (used with an explicit env_stride)
     double dbss_eps = 0.0;                        // > 0: dynamic block state selection, truncation error target per bond
     int dbss_dmin = 0;                            // DBSS lower bound on the kept states
     int split_k = 0;                              // split-K parts of phase 2 of H_eff psi (0 = automatic)
@@ -289,7 +290,7 @@ struct Engine {
     bool keep_env_stack = true;
     // environment-stack memory path of dmrg_sweep (row "m"): checkpoints every env_stride bonds, the blocks between two
     // checkpoints are recomputed when a pass enters that segment; checkpoints optionally spilled to pinned host memory
-    int env_stride = 1;
+    int env_stride = 1, env_stride2 = 1;
     bool env_spill = false;
     HostPool host_pool;
     cudaStream_t copy_stream = nullptr;

@@ -495,13 +495,27 @@ void Engine::plan_env_policy(int D) {
     const double budget = opt.hbm_budget_bytes > 0 ? (double)opt.hbm_budget_bytes : 0.55 * ((double)free_b + (double)g_device_bytes_env(*this));
     const double host_budget = opt.host_budget_bytes > 0 ? (double)opt.host_budget_bytes : 64.0 * (double)(1ull << 30);
     env_spill = false;
-    if (opt.env_stride > 0) { env_stride = opt.env_stride; env_spill = opt.host_spill != 0; return; }
+    env_stride2 = 1;
+    if (opt.env_stride > 0) { env_stride = opt.env_stride; env_stride2 = std::max(1, opt.env_stride2); env_spill = opt.host_spill != 0; return; }
     if (total <= budget) { env_stride = 1; return; }
     if (opt.host_spill) {
         // checkpoints on the host, the segment being consumed (stride blocks) plus the block being produced on the device
         int s = 1;
         while (s < k && total / s > host_budget) ++s;
-        if ((s + 1) * bmax > budget) throw Error(-3, "environment stack: one segment between host checkpoints exceeds the device budget");
+        env_stride2 = 1;
+        if ((s + 1) * bmax > budget) {
+            // a whole segment does not fit: second checkpoint level inside the segment (s / s2 kept blocks + s2 of the
+            // current sub-segment + the block being produced and the restored checkpoint)
+            int best2 = 0;
+            double need2 = 0.0;
+            for (int q = 2; q < s; ++q) {
+                const double need = ((s + q - 1) / q + q + 2) * bmax;
+                if (!best2 || need < need2) { best2 = q; need2 = need; }
+            }
+            if (!best2 || need2 > budget) throw Error(-3, "environment stack: one segment between host checkpoints exceeds the device budget");
+            env_stride = s; env_stride2 = best2; env_spill = true;
+            return;
+        }
         // fewer, larger segments while they stay within half the budget (at most 8 blocks): pinning host memory for a
         // checkpoint costs more than recomputing a block (measured, config 4 at D = 2048: stride 6 -> 319 s, stride 2 -> 346 s
         // for the first sweep; later sweeps reuse the pinned pool)
@@ -567,7 +581,15 @@ Block& Engine::need_left(int b) {
     if (L.find(c) == L.end()) L[0] = empty_block('L', k, mps);
     make_resident(*this, *L.at(c));
     const double t0 = wall();
-    for (int j = c; j < b; ++j) L[j + 1] = grow(*L.at(j), ham, mps, mode_L(j + 1), *this);
+    // second checkpoint level (env_stride2 > 1): of the blocks between the checkpoint and the target only every
+    // env_stride2-th one and the target's own sub-segment stay; the rest is erased as soon as it has produced its
+    // successor and is recomputed from the nearest kept block when the pass gets there
+    const int s2 = std::max(1, env_stride2);
+    const int keep_above = ((b - 1) / s2) * s2;                       // sub-segment of the target: (keep_above, b]
+    for (int j = c; j < b; ++j) {
+        L[j + 1] = grow(*L.at(j), ham, mps, mode_L(j + 1), *this);
+        if (j != c && j % s2 != 0 && j <= keep_above) L.erase(j);
+    }
     t_regrow += wall() - t0;
     return *L.at(b);
 }
@@ -579,7 +601,12 @@ Block& Engine::need_right(int b) {
     if (R.find(c) == R.end()) R[k] = empty_block('R', k, mps);
     make_resident(*this, *R.at(c));
     const double t0 = wall();
-    for (int j = c; j > b; --j) R[j - 1] = grow(*R.at(j), ham, mps, mode_R(j - 1), *this);
+    const int s2 = std::max(1, env_stride2);
+    const int keep_below = (b / s2 + 1) * s2;                         // sub-segment of the target: [b, keep_below)
+    for (int j = c; j > b; --j) {
+        R[j - 1] = grow(*R.at(j), ham, mps, mode_R(j - 1), *this);
+        if (j != c && j % s2 != 0 && j >= keep_below) R.erase(j);
+    }
     t_regrow += wall() - t0;
     return *R.at(b);
 }

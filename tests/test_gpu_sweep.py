@@ -103,7 +103,8 @@ def test_config1_untruncated_reaches_golden_fci(lib):
 
 
 @pytest.mark.parametrize("opts", [dict(env_stride=3), dict(env_stride=2, host_spill=1), dict(env_stride=1, host_spill=1),
-                                  dict(env_stride=4, host_spill=1)])
+                                  dict(env_stride=4, host_spill=1), dict(env_stride=6, env_stride2=2, host_spill=1),
+                                  dict(env_stride=9, env_stride2=3)])
 def test_sweep_env_checkpoints_and_host_spill_are_bit_identical(lib, opts):
     """Environment-stack memory path: keeping only every env_stride-th block (the others recomputed when
     a pass reaches them) and spilling the checkpoints to pinned host memory must not change a single bit of a sweep,
