@@ -66,3 +66,13 @@ def test_golden_config1_internal_pins():
     occ = np.array(vals["natural_occupations"])
     assert abs(occ.sum() - 10.0) < 1e-6 and abs(vals["trace_gamma"][0] - 10.0) < 1e-9
     assert np.abs(occ + occ[::-1] - 2.0).max() < 1e-6
+
+
+def test_stored_traffic_is_labelled_and_workload_specific():
+    """roofline.traffic comes from the tracked ncu summary (commit + command + number of launches of one step) and only
+    for the workload it was captured on."""
+    import bench
+    t, note = bench.stored_traffic(4, 4096, 26)
+    assert t is not None and t > 5.0e10 and "commit" in note and "launches" in note
+    assert bench.stored_traffic(4, 2048, 26) == (None, None)
+    assert bench.stored_traffic(5, 4096, 40) == (None, None)
