@@ -77,24 +77,58 @@ __global__ void __launch_bounds__(256) scale_kernel(double a, double* __restrict
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) x[i] *= a;
 }
 
-// one CTA per psi block (grid-strided over blocks); the diagonals of the operator blocks are staged in registers per item
+// one CTA per psi block (grid-strided over blocks).  The diagonals of the operator blocks of a tile of items are
+// gathered once into shared memory (R + C strided loads per item instead of two per element and item), then every
+// element adds  c_t l_t[i] r_t[j]  in item order (the same summation order as a plain loop over the items).
+constexpr int DIAG_SH = 6000;                      // doubles of staging: items per tile = DIAG_SH / (R + C), at most 16
 __global__ void __launch_bounds__(256) heff_diag_kernel(double* __restrict__ d, int nblocks, const int64_t* __restrict__ off,
                                                         const int* __restrict__ rows, const int* __restrict__ cols,
                                                         const int* __restrict__ ptr, const DiagItemK* __restrict__ items) {
+    __shared__ double sh[DIAG_SH];
+    __shared__ double sc[16];
     for (int b = blockIdx.x; b < nblocks; b += gridDim.x) {
         const int R = rows[b], Cc = cols[b];
         const int64_t total = (int64_t)R * Cc;
-        for (int64_t e = threadIdx.x; e < total; e += blockDim.x) {
-            const int i = (int)(e / Cc), j = (int)(e % Cc);
-            double s = 0.0;
-            for (int t = ptr[b]; t < ptr[b + 1]; ++t) {
-                const DiagItemK it = items[t];
-                const double l = it.ml ? it.ml[(size_t)i * (it.ldl + 1)] : 1.0;
-                const double r = it.mr ? it.mr[(size_t)j * (it.ldr + 1)] : 1.0;
-                s += it.c * l * r;
+        double* out = d + off[b];
+        const int t0 = ptr[b], t1 = ptr[b + 1];
+        if (t1 == t0) { for (int64_t e = threadIdx.x; e < total; e += blockDim.x) out[e] = 0.0; continue; }
+        int DT = DIAG_SH / (R + Cc);
+        if (DT > 16) DT = 16;
+        if (DT < 1) {                              // a block too wide for the staging buffer: direct loop
+            for (int64_t e = threadIdx.x; e < total; e += blockDim.x) {
+                const int i = (int)(e / Cc), j = (int)(e % Cc);
+                double s = 0.0;
+                for (int t = t0; t < t1; ++t) {
+                    const DiagItemK it = items[t];
+                    const double l = it.ml ? it.ml[(size_t)i * (it.ldl + 1)] : 1.0;
+                    const double r = it.mr ? it.mr[(size_t)j * (it.ldr + 1)] : 1.0;
+                    s += it.c * l * r;
+                }
+                out[e] = s;
             }
-            d[off[b] + e] = s;
+            continue;
         }
+        for (int tb = t0; tb < t1; tb += DT) {
+            const int nt = min(DT, t1 - tb);
+            __syncthreads();                       // previous tile (and previous block) fully consumed
+            for (int q = threadIdx.x; q < nt * (R + Cc); q += blockDim.x) {
+                const int t = q / (R + Cc), x = q % (R + Cc);
+                const DiagItemK& it = items[tb + t];
+                double v;
+                if (x < R) v = it.ml ? it.ml[(size_t)x * (it.ldl + 1)] : 1.0;
+                else       v = it.mr ? it.mr[(size_t)(x - R) * (it.ldr + 1)] : 1.0;
+                sh[q] = v;
+            }
+            if (threadIdx.x < nt) sc[threadIdx.x] = items[tb + threadIdx.x].c;
+            __syncthreads();
+            for (int64_t e = threadIdx.x; e < total; e += blockDim.x) {
+                const int i = (int)(e / Cc), j = (int)(e % Cc);
+                double s = tb == t0 ? 0.0 : out[e];
+                for (int t = 0; t < nt; ++t) s += sc[t] * sh[t * (R + Cc) + i] * sh[t * (R + Cc) + R + j];
+                out[e] = s;
+            }
+        }
+        __syncthreads();
     }
 }
 
