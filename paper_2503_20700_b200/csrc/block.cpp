@@ -511,7 +511,7 @@ void lincomb(Block& blk, const std::vector<LinSpec>& specs, bool accumulate, Eng
         int src_stack = -1;
         for (const LinSpec* s : kv.second)
             for (const LinItem& it : s->items) {
-                const int st = blk.get(it.src).stack;
+                const int st = it.stack >= 0 ? it.stack : blk.get(it.src).stack;
                 if (src_stack >= 0 && st != src_stack) throw std::logic_error("lincomb: sources span two stacks");
                 src_stack = st;
             }
@@ -529,7 +529,7 @@ void lincomb(Block& blk, const std::vector<LinSpec>& specs, bool accumulate, Eng
         std::vector<double> W((size_t)n_dst * ldw, 0.0);
         for (const LinSpec* s : kv.second) {
             const int r = blk.get(s->dst).row;
-            for (const LinItem& it : s->items) W[(size_t)r * ldw + blk.get(it.src).row] += it.coef;
+            for (const LinItem& it : s->items) W[(size_t)r * ldw + (it.row >= 0 ? it.row : blk.get(it.src).row)] += it.coef;
         }
         keep.emplace_back();
         keep.back().upload(W, eng.stream);

@@ -187,7 +187,7 @@ struct OpBlockView { int out; const double* ptr; int ld; bool trans; int rows, c
 // stored (ld = d_in) or stored^T (stored [d_in x d_out], ld = d_out, trans = true)
 bool op_block(const Block& blk, const OpRef& op, bool trans, int in, OpBlockView& v);
 
-struct LinItem { double coef; Label src; };
+struct LinItem { double coef; Label src; int stack = -1, row = -1; };   // stack / row: optional hint (skips the label lookup)
 struct LinSpec { Label dst; std::vector<LinItem> items; };
 // dst = (accumulate ? dst : 0) + sum coef * src for every spec, as one stack GEMM per (kind, class) pair
 void lincomb(Block& blk, const std::vector<LinSpec>& specs, bool accumulate, Engine& eng);

@@ -34,56 +34,82 @@ void make_temps(const Ham& ham, Block& X, const Dot& dot, const std::vector<int>
     std::vector<int> pool = dot.so;
     pool.insert(pool.end(), far.begin(), far.end());
     std::sort(pool.begin(), pool.end());
+    // destinations first (cheap), then the integral-weighted source lists on the host threads: at k = 82 that is ~10^7
+    // lookups of (pq|rs) per bond.  Dense (stack, row) tables of the stored A / B / C operators replace the label lookups.
+    const int nso = 2 * X.k;
+    struct Src { int stack, row; };
+    std::vector<Src> tA((size_t)nso * nso, Src{-1, -1}), tB((size_t)nso * nso, Src{-1, -1}), tC(nso, Src{-1, -1});
+    for (const auto& kv : X.ops) {
+        const int kind = (int)(kv.first >> 24), a = (int)((kv.first >> 16) & 255), b = (int)((kv.first >> 8) & 255);
+        if (kind == K_A) tA[(size_t)a * nso + b] = {kv.second.stack, kv.second.row};
+        else if (kind == K_B) tB[(size_t)a * nso + b] = {kv.second.stack, kv.second.row};
+        else if (kind == K_C) tC[a] = {kv.second.stack, kv.second.row};
+    }
+    auto shift = [](const Label& x, int& a, int& b) { op_shift(x, a, b); };
     std::vector<LinSpec> specs;
-    auto same_shift = [](const Label& x, const Label& y) {
-        int a, b, c, d;
-        op_shift(x, a, b); op_shift(y, c, d);
-        return a == c && b == d;
-    };
     if (X.mode == 'N') {
         for (size_t a = 0; a < pool.size(); ++a)
             for (size_t b = a + 1; b < pool.size(); ++b) {
-                const int P = pool[a], Q = pool[b];
-                if (!dot.has(P) && !dot.has(Q)) continue;
-                LinSpec s; s.dst = L2(K_Pt, P, Q);             // (P_PQ)^T = -sum_{R<S} w_PQRS A_RS
-                for (size_t i = 0; i < Xin.size(); ++i)
-                    for (size_t j = i + 1; j < Xin.size(); ++j) {
-                        const Label src = L2(K_A, Xin[i], Xin[j]);
-                        if (same_shift(src, s.dst)) s.items.push_back({-ham.w(P, Q, Xin[i], Xin[j]), src});
-                    }
+                if (!dot.has(pool[a]) && !dot.has(pool[b])) continue;
+                LinSpec s; s.dst = L2(K_Pt, pool[a], pool[b]);   // (P_PQ)^T = -sum_{R<S} w_PQRS A_RS
                 specs.push_back(s);
             }
         for (int P : pool)
             for (int S : pool) {
                 if (!dot.has(P) && !dot.has(S)) continue;
                 LinSpec s; s.dst = L2(K_Q, P, S);              // Q_PS = sum_{QR} w_PQRS B_QR
-                for (int Q : Xin)
-                    for (int R : Xin) {
-                        const Label src = L2(K_B, Q, R);
-                        if (same_shift(src, s.dst)) s.items.push_back({ham.w(P, Q, R, S), src});
-                    }
                 specs.push_back(s);
             }
     }
+    const size_t n_two = specs.size();
     for (int P : far) {
         for (size_t a = 0; a < dot.so.size(); ++a)
-            for (size_t b = a + 1; b < dot.so.size(); ++b) {
-                const int R = dot.so[a], S = dot.so[b];
-                LinSpec s; s.dst = L3(K_U, P, R, S);           // U_{P;RS} = sum_Q w_PQRS a+_Q
-                for (int Q : Xin) { const double w = ham.w(P, Q, R, S); if (w != 0.0) s.items.push_back({w, L1(K_C, Q)}); }
-                if (!s.items.empty()) specs.push_back(s);
-            }
+            for (size_t b = a + 1; b < dot.so.size(); ++b) { LinSpec s; s.dst = L3(K_U, P, dot.so[a], dot.so[b]); specs.push_back(s); }   // U_{P;RS} = sum_Q w_PQRS a+_Q
         for (int Q : dot.so)
-            for (int R : dot.so) {
-                LinSpec s; s.dst = L3(K_V, P, Q, R);           // V_{P;QR} = sum_S w_PQRS a+_S
-                for (int S : Xin) { const double w = ham.w(P, Q, R, S); if (w != 0.0) s.items.push_back({w, L1(K_C, S)}); }
-                if (!s.items.empty()) specs.push_back(s);
-            }
+            for (int R : dot.so) { LinSpec s; s.dst = L3(K_V, P, Q, R); specs.push_back(s); }                                                // V_{P;QR} = sum_S w_PQRS a+_S
     }
+#pragma omp parallel for schedule(dynamic, 8) if (specs.size() > 64)
+    for (long j = 0; j < (long)specs.size(); ++j) {
+        LinSpec& s = specs[j];
+        int dn, ds, sn, ss;
+        shift(s.dst, dn, ds);
+        if (s.dst.kind == K_Pt) {
+            const int P = s.dst.a, Q = s.dst.b;
+            for (size_t i = 0; i < Xin.size(); ++i)
+                for (size_t q = i + 1; q < Xin.size(); ++q) {
+                    const Label src = L2(K_A, Xin[i], Xin[q]);
+                    shift(src, sn, ss);
+                    if (sn != dn || ss != ds) continue;
+                    const Src t = tA[(size_t)Xin[i] * nso + Xin[q]];
+                    s.items.push_back({-ham.w(P, Q, Xin[i], Xin[q]), src, t.stack, t.row});
+                }
+        } else if (s.dst.kind == K_Q) {
+            const int P = s.dst.a, S = s.dst.b;
+            for (int Q : Xin)
+                for (int R : Xin) {
+                    const Label src = L2(K_B, Q, R);
+                    shift(src, sn, ss);
+                    if (sn != dn || ss != ds) continue;
+                    const Src t = tB[(size_t)Q * nso + R];
+                    s.items.push_back({ham.w(P, Q, R, S), src, t.stack, t.row});
+                }
+        } else if (s.dst.kind == K_U) {
+            const int P = s.dst.a, R = s.dst.b, S = s.dst.c;
+            for (int Q : Xin) { const double w = ham.w(P, Q, R, S); if (w != 0.0) s.items.push_back({w, L1(K_C, Q), tC[Q].stack, tC[Q].row}); }
+        } else {
+            const int P = s.dst.a, Q = s.dst.b, R = s.dst.c;
+            for (int S : Xin) { const double w = ham.w(P, Q, R, S); if (w != 0.0) s.items.push_back({w, L1(K_C, S), tC[S].stack, tC[S].row}); }
+        }
+    }
+    // one-index combinations without any source are not stored (their absence is how the generator skips them)
+    std::vector<LinSpec> kept;
+    kept.reserve(specs.size());
+    for (size_t j = 0; j < specs.size(); ++j)
+        if (j < n_two || !specs[j].items.empty()) kept.push_back(std::move(specs[j]));
     std::vector<Label> labels;
-    for (const LinSpec& s : specs) labels.push_back(s.dst);
+    for (const LinSpec& s : kept) labels.push_back(s.dst);
     X.allocate(labels, true);
-    lincomb(X, specs, false, eng);
+    lincomb(X, kept, false, eng);
 }
 
 // ---------------------------------------------------------------------------------------------------------------
