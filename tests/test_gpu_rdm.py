@@ -167,3 +167,36 @@ def test_rdm12_config4_chain_partition_points_agree(lib):
     for (g1, G1) in res[1:]:
         assert np.abs(g - g1).max() <= TOL and np.abs(G - G1).max() <= TOL
     _invariants(g, G, n)
+
+
+def test_rdm12_and_diag_into_device_buffers_on_the_callers_stream(lib):
+    """`where = DMRG_DEVICE`: dmrg_rdm12 and dmrg_heff_diag write into caller device buffers on the caller's stream
+    (ordered after its pending work) and agree with the host-buffer results."""
+    import torch
+    k, n, s2, D = 6, 6, 0, 12
+    h, eri = random_dense(k, 31)
+    mps = random_mps(k, n, s2, D, seed=14, gauge="R")
+    ctx = lib.dmrg_create(k, n, s2, h, eri)
+    try:
+        lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, s2)
+        g0, G0 = lib.dmrg_rdm12(ctx, k, True)
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            gd = torch.full((k, k), 7.0, dtype=torch.float64, device="cuda")      # pending work on the buffers
+            Gd = torch.full((k, k, k, k), 7.0, dtype=torch.float64, device="cuda")
+            lib.dmrg_rdm12(ctx, k, True, out=(gd, Gd))
+            g1, G1 = gd.cpu().numpy(), Gd.cpu().numpy()
+        assert np.array_equal(g0, g1) and np.array_equal(G0, G1)
+        i = 2
+        lib.dmrg_mps_import(ctx, mps_to_blob_arrays(random_mps(k, n, s2, D, seed=15, gauge="LR:%d" % i)), k, n, s2)
+        lib.dmrg_prepare_bond(ctx, i)
+        nnz, _ = lib.dmrg_heff_layout(ctx, i)
+        dh = np.zeros(nnz)
+        lib.dmrg_heff_diag(ctx, i, dh)
+        with torch.cuda.stream(st):
+            dd = torch.full((nnz,), 3.0, dtype=torch.float64, device="cuda")
+            lib.dmrg_heff_diag(ctx, i, dd)
+            d1 = dd.cpu().numpy()
+        assert np.array_equal(dh, d1)
+    finally:
+        lib.dmrg_destroy(ctx)
