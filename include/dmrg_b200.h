@@ -222,6 +222,19 @@ int dmrg_grouped_gemm(int ntasks, const int64_t* c_ptr, const int32_t* ldc, cons
 int dmrg_stack_dots(const double* S, int64_t lds, int nrows, const double* M, int64_t ldm, int nc, int64_t K, double* E,
                     int ldE, double* ms, void* cuda_stream);
 
+/* Allocation-free variant of dmrg_stack_dots for callers that cannot call cudaMalloc (CUDA graph capture, tight serving
+ * loops, harnesses that forbid allocation): same operation, same kernels, same argument meaning; the span partial sums
+ * live in one static device array of DMRG_STACK_DOTS_NOALLOC_MAX_SCRATCH doubles (8 MiB, held by every GPU that loads the
+ * library until exit).  Calls no cudaMalloc / cudaFree / allocating library routine, creates no events and does not
+ * synchronise: the launches are asynchronous on `cuda_stream`.  Limit: the scratch need is nspans * nrows * nc doubles
+ * with nspans <= ceil(2368 / ceil(nrows / 32)) K spans; every nc <= 8 with nrows <= 32768 fits; a problem that needs more
+ * returns DMRG_ENOMEM (nothing launched) - use dmrg_stack_dots then.  All calls on a device share the array: calls that overlap on
+ * the GPU (different streams or host threads) race; order them on one stream.  Nothing in the array needs clearing
+ * between calls (every partial sum read was written by the same call). */
+#define DMRG_STACK_DOTS_NOALLOC_MAX_SCRATCH (1 << 20)
+int dmrg_stack_dots_noalloc(const double* S, int64_t lds, int nrows, const double* M, int64_t ldm, int nc, int64_t K,
+                            double* E, int ldE, void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

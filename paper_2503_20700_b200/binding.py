@@ -60,7 +60,7 @@ class dmrg_sweep_result(C.Structure):
 EXPORTS = ["dmrg_default_options", "dmrg_create", "dmrg_destroy", "dmrg_last_error", "dmrg_mps_import",
            "dmrg_mps_export", "dmrg_prepare_bond", "dmrg_heff_layout", "dmrg_heff_apply", "dmrg_heff_diag",
            "dmrg_heff_stats", "dmrg_sweep", "dmrg_solve", "dmrg_sweep_stats", "dmrg_rdm12", "dmrg_rdm_stats", "dmrg_launch_count", "dmrg_flops_total", "dmrg_device_bytes",
-           "dmrg_grouped_gemm", "dmrg_stack_dots"]
+           "dmrg_grouped_gemm", "dmrg_stack_dots", "dmrg_stack_dots_noalloc"]
 
 lib.dmrg_last_error.restype = C.c_char_p
 lib.dmrg_last_error.argtypes = [C.c_void_p]
@@ -278,6 +278,20 @@ def dmrg_grouped_gemm(tasks, segs, stream=None, generic=False):
     return ms.value
 
 
+def dmrg_stack_dots_noalloc(S_ptr, lds, nrows, M_ptr, ldm, nc, K, E_ptr, ldE, stream=None):
+    """Allocation-free variant of dmrg_stack_dots (static device scratch of DMRG_STACK_DOTS_NOALLOC_MAX_SCRATCH doubles):
+    asynchronous on `stream`, no timing.  Raises DmrgError(DMRG_ENOMEM) when the problem exceeds the static scratch."""
+    rc = lib.dmrg_stack_dots_noalloc(C.c_void_p(S_ptr), C.c_int64(lds), int(nrows), C.c_void_p(M_ptr), C.c_int64(ldm), int(nc),
+                                     C.c_int64(K), C.c_void_p(E_ptr), int(ldE), C.c_void_p(stream or 0))
+    if rc == DMRG_ENOMEM:
+        raise DmrgError(rc, "dmrg_stack_dots_noalloc: problem needs more than the static scratch (%d doubles); use dmrg_stack_dots"
+                        % DMRG_STACK_DOTS_NOALLOC_MAX_SCRATCH)
+    if rc != 0:
+        raise DmrgError(rc, "dmrg_stack_dots_noalloc failed")
+    return rc
+
+
+DMRG_STACK_DOTS_NOALLOC_MAX_SCRATCH = 1 << 20
 _bench_lib = None
 
 
