@@ -67,7 +67,7 @@ def parse_args():
     ap.add_argument("--env-stride2", type=int, default=0)
     ap.add_argument("--hbm-budget-gb", type=float, default=0.0)
     ap.add_argument("--host-budget-gb", type=float, default=0.0)
-    ap.add_argument("--cpu-baseline", type=int, default=1)
+    ap.add_argument("--cpu-baseline", type=int, default=2, help="1: oracle H_eff psi sample on the config-4 Hamiltonian; 2: also the oracle's sweep + RDM pass on config 1 (concurrently, another process); 0: none")
     ap.add_argument("--sample-config", type=int, default=4, help="config of the oracle's bounded sample (default: the metric's own Hamiltonian)")
     ap.add_argument("--sample-D", type=int, default=48, help="bond dimension of the oracle's bounded sample")
     ap.add_argument("--sweep-D", type=int, default=2048, help="bond dimension of the --big sweeps")
@@ -151,7 +151,7 @@ def _oracle_env(job):
     return odmrg.build_left(mps, oham, i)[-1] if side == "L" else odmrg.build_right(mps, oham, i + 2)[i + 2]
 
 
-def oracle_sample(args, steps, warmup):
+def oracle_sample(args, steps, warmup, with_sweep=False):
     """The oracle, as it stands, on a bounded sample of the metric's workload: H_eff psi at the mid-chain bond of the
     SAME Hamiltonian (BASELINE config 4, k = 54, 9 279-term list class) at the largest bond dimension whose run fits the
     time box (--sample-D); its own environments come from its own renormalisation (untimed, the two sides in two
@@ -161,8 +161,10 @@ def oracle_sample(args, steps, warmup):
     cfg, D, i, mps, _ = build_workload(args.sample_config, args.sample_D, -1)
     oham = odmrg.Ham(cfg["h"], cfg["eri"])
     t0 = time.perf_counter()
-    with mp.get_context("fork").Pool(2) as pool:
-        oL, oR = pool.map(_oracle_env, [("L", args.sample_config, args.sample_D, i), ("R", args.sample_config, args.sample_D, i)])
+    pool = mp.get_context("fork").Pool(3 if with_sweep else 2)
+    # the oracle's own sweep + RDM pass on config 1 runs in a third process beside this sample (other cores)
+    sweep_job = pool.apply_async(oracle_small_sweep_rdm) if with_sweep else None
+    oL, oR = pool.map(_oracle_env, [("L", args.sample_config, args.sample_D, i), ("R", args.sample_config, args.sample_D, i)])
     H = odmrg.Heff(oL, oR, oham, i)
     t_env = time.perf_counter() - t0
     x = np.random.default_rng(1).normal(size=H.nnz)
@@ -187,6 +189,10 @@ def oracle_sample(args, steps, warmup):
                        "flops = the oracle's own per-block GEMM count" %
                        (cfg["name"], cfg["k"], D, i, H.nnz, len(H.terms), steps, t_env), ms_per_step=sec * 1e3, f_alg=f_alg,
                 setup_seconds=t_env)
+    if sweep_job is not None:
+        info["config1_sweep_rdm"] = sweep_job.get()
+    pool.close()
+    pool.join()
     return f_alg / sec / 1e12, info
 
 
@@ -203,7 +209,8 @@ def oracle_small_sweep_rdm():
     g, G = odmrg.rdm12(cfg["h"], cfg["eri"], eng.mps, True)   # right-canonical, centre on site 0 after a full sweep
     t2 = time.perf_counter()
     return {"workload": "%s D=64" % cfg["name"], "s_per_sweep": t1 - t0, "matvecs": int(sum(b["n_matvec"] for b in r["bonds"])),
-            "rdm12_seconds": t2 - t1, "trace_gamma": float(np.trace(g))}
+            "rdm12_seconds": t2 - t1, "trace_gamma": float(np.trace(g)),
+            "note": "oracle/dmrg.py SweepEngine (Davidson tol 1e-7) first sweep from the seeded random MPS, then oracle rdm12 on the swept MPS; one process"}
 
 
 def max_over_ranks(x, device):
@@ -500,10 +507,8 @@ def run_ours(args):
     if args.extras:
         line["extras"] = time_small_extras(P, torch, peaks, args.extras)
     if args.cpu_baseline and world == 1:
-        v, info = oracle_sample(args, 1, 0)
+        v, info = oracle_sample(args, 1, 0, with_sweep=args.cpu_baseline > 1)
         line["cpu_baseline"] = dict(info, value=v, unit=UNIT)
-        if args.cpu_baseline > 1:
-            line["cpu_baseline"]["config1_sweep_rdm"] = oracle_small_sweep_rdm()
     print(json.dumps(line))
 
 
