@@ -1022,11 +1022,16 @@ def rdm12(h, eri, mps_in, want_2rdm=True):
     g2 = np.zeros((n_so,) * 4) if want_2rdm else None
     site_of = lambda P: P >> 1
 
+    site_mats = {}
+
     def site_mat(ops):
-        m = np.eye(4)
-        for (P, dag) in ops:
-            m = m @ (site_ann(P).T if dag else site_ann(P))
-        return m
+        key = tuple((P & 1, dag) for (P, dag) in ops)         # the 4x4 matrix depends only on spin and dagger
+        if key not in site_mats:
+            m = np.eye(4)
+            for (P, dag) in ops:
+                m = m @ (site_ann(P).T if dag else site_ann(P))
+            site_mats[key] = m
+        return site_mats[key]
 
     def right_op(RB, ops):
         if not ops:
@@ -1068,11 +1073,25 @@ def rdm12(h, eri, mps_in, want_2rdm=True):
                 if min(site_of(P), site_of(S)) == c:
                     add_string(((P, True), (S, False)), (P, S))
         if want_2rdm:
+            # all (P<Q, S<R) whose second-smallest site is c, i.e. at most one operator left of c and at least two on
+            # sites <= c.  Integer bookkeeping only: the pairs are binned by (#left of c, #on c) and only admissible bins
+            # are combined (the same set as scanning every quadruple and testing sorted(sites)[1] == c; each string is
+            # an independent assignment, so the visiting order does not matter).  Strings that change 2Sz are skipped:
+            # their expectation value in an Sz eigenstate is zero (g2 starts at zero).
+            bins = {}
             for P in range(n_so):
                 for Q in range(P + 1, n_so):
-                    for S in range(n_so):
-                        for R in range(S + 1, n_so):
-                            if sorted((site_of(P), site_of(Q), site_of(R), site_of(S)))[1] == c:
+                    nl = (site_of(P) < c) + (site_of(Q) < c)
+                    nc = (site_of(P) == c) + (site_of(Q) == c)
+                    if nl <= 1:
+                        bins.setdefault((nl, nc), []).append((P, Q, spin_of(P) + spin_of(Q)))
+            for (nl1, nc1), cre in bins.items():
+                for (nl2, nc2), ann in bins.items():
+                    if nl1 + nl2 > 1 or nl1 + nl2 + nc1 + nc2 < 2:
+                        continue
+                    for (P, Q, sc) in cre:
+                        for (S, R, sa) in ann:
+                            if sc == sa:
                                 add_string(((P, True), (Q, True), (R, False), (S, False)), (P, Q, R, S))
         # ---- evaluate ------------------------------------------------------------------------------------------
         for rops, items in groups.items():

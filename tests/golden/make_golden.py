@@ -21,9 +21,10 @@ Nothing here imports the CUDA package.  Each file records the command that wrote
       NSWEEPS two-site sweeps (readings S12-S18, Davidson tolerance 1e-10 as in S13) from oracle.dmrg.SweepEngine on
       random_mps(seed = config seed + 1000, gauge R, D = DINIT or D).
 
-  python tests/golden/make_golden.py rdm CFG D
+  python tests/golden/make_golden.py rdm CFG D [NSAMPLE]
       rdm_cfgC_DD.npz - gamma and Gamma (Eq. 9-10, readings S2 / S20) of random_mps(seed = 900 + CFG,
-      gauge R) from oracle.dmrg.rdm12.
+      gauge R) from oracle.dmrg.rdm12; with NSAMPLE (k = 54: Gamma has 8.5e6 entries) a seeded sample of Gamma plus
+      the full-array scalars sum Gamma^2 and sum_pr Gamma_pprr instead of the whole array.
 
 CFG 1-5 are BASELINE.json's configs; CFG 6 is the open-shell second workload of synth/ (Fe-S-like CAS(29,20), 2Sz = 5;
 SURVEY.md 8(f) rank 4).
@@ -110,16 +111,33 @@ def golden_sweep(cid, D, nsweeps, Dinit):
     print(note, flush=True)
 
 
-def golden_rdm(cid, D):
+def golden_rdm(cid, D, nsample=0):
+    """nsample > 0 (large k: Gamma has k^4 entries): store gamma, a seeded sample of nsample entries of Gamma (flat indices
+    from default_rng(77)), and the full-array scalars sum Gamma^2 and sum_pr Gamma_pprr instead of Gamma itself."""
     cfg = make_config(cid)
     k, n = cfg["k"], cfg["n_elec"]
     mps = random_mps(k, n, cfg["two_sz"], D, seed=900 + cid, gauge="R")
     t0 = time.time()
-    g, G = odmrg.rdm12(cfg["h"], cfg["eri"], mps, True)
-    note = ("written by `python tests/golden/make_golden.py rdm %d %d` from oracle.dmrg.rdm12; oracle time %.0f s on "
-            "%d host cores" % (cid, D, time.time() - t0, os.cpu_count()))
-    np.savez_compressed(os.path.join(HERE, "rdm_cfg%d_D%d.npz" % (cid, D)), gamma=g, Gamma=G, D=D, config=cid,
-                        mps_seed=900 + cid, note=note)
+    move = odmrg._move_centre_right
+
+    def progress(m, c):                                     # progress line per centre (the pass takes hours at k = 54)
+        print("  centre %d done, %.0f s" % (c, time.time() - t0), flush=True)
+        return move(m, c)
+    odmrg._move_centre_right = progress
+    try:
+        g, G = odmrg.rdm12(cfg["h"], cfg["eri"], mps, True)
+    finally:
+        odmrg._move_centre_right = move
+    note = ("written by `python tests/golden/make_golden.py rdm %d %d%s` from oracle.dmrg.rdm12; oracle time %.0f s on "
+            "%d host cores" % (cid, D, " %d" % nsample if nsample else "", time.time() - t0, os.cpu_count()))
+    out = dict(gamma=g, D=D, config=cid, mps_seed=900 + cid, note=note)
+    if nsample:
+        idx = np.sort(np.random.default_rng(77).choice(G.size, size=nsample, replace=False))
+        out.update(sample_idx=idx, sample_val=G.ravel()[idx], sum_sq=float(np.sum(G * G)),
+                   trace2=float(np.einsum("pprr->", G)))
+    else:
+        out["Gamma"] = G
+    np.savez_compressed(os.path.join(HERE, "rdm_cfg%d_D%d.npz" % (cid, D)), **out)
     print(note, flush=True)
 
 
@@ -133,7 +151,7 @@ def main():
     elif what == "sweep":
         golden_sweep(a[0], a[1], a[2], a[3] if len(a) > 3 else a[1])
     elif what == "rdm":
-        golden_rdm(a[0], a[1])
+        golden_rdm(a[0], a[1], a[2] if len(a) > 2 else 0)
     else:
         raise SystemExit(__doc__)
 
