@@ -1,8 +1,8 @@
 """CUDA path vs stored oracle results (tests/golden/, written by tests/golden/make_golden.py from oracle/ alone) at
 sizes the plain Python oracle only reaches offline: H_eff psi and diag(H_eff) on the k = 54 (BASELINE config 4) and
 k = 82 (config 5) Hamiltonians - the 9 279 / 18 715-term lists with the N/C-mode switch on either side of the bond -,
-two-site sweeps of configs 2 and 3, and the 1-/2-RDMs of configs 2 and 3 at bond dimensions where operator classes
-have many right-hand sides and several K spans.  Inputs are rebuilt here from the same seeded generators (synth/).
+two-site sweeps of configs 2 and 3, the 1-/2-RDMs of configs 2 and 3 at bond dimensions where operator classes
+have many right-hand sides and several K spans, and the 1-/2-RDMs on the k = 54 chain (gamma and a seeded sample of Gamma).  Inputs are rebuilt here from the same seeded generators (synth/).
 Tolerances (BASELINE.json north_star): H_eff psi rel. L2 <= 1e-11, RDM max-abs <= 1e-10, sweep energies <= 1e-8 Eh."""
 import glob
 import json
@@ -25,6 +25,7 @@ def test_golden_files_present():
     """configs 4 and 5 must have an H_eff golden, configs 2 and 3 a sweep and an RDM golden."""
     for c in (4, 5):
         assert _files("heff_cfg%d_D*.npz" % c)
+    assert _files("rdm_cfg4_D*.npz")                              # k = 54: the half-chain RDM pass vs the oracle's pass
     for c in (2, 3, 6):                                           # 6: the open-shell second workload (2Sz = 5, odd N)
         assert _files("sweep_cfg%d_D*.json" % c) and _files("rdm_cfg%d_D*.npz" % c)
 
