@@ -16,10 +16,11 @@ Nothing here imports the CUDA package.  Each file records the command that wrote
       inputs for the CUDA library.  The plain Python oracle cannot reach the configs' own D (4096 / 2048) on k = 54 /
       82 in bounded time; the files say which D it did reach and how long that took.
 
-  python tests/golden/make_golden.py sweep CFG D NSWEEPS [DINIT]
+  python tests/golden/make_golden.py sweep CFG D NSWEEPS [DINIT [NBONDS]]
       sweep_cfgC_DD.json - per-bond Davidson energies, kept bond dimension, sector count and truncation error of
       NSWEEPS two-site sweeps (readings S12-S18, Davidson tolerance 1e-10 as in S13) from oracle.dmrg.SweepEngine on
-      random_mps(seed = config seed + 1000, gauge R, D = DINIT or D).
+      random_mps(seed = config seed + 1000, gauge R, D = DINIT or D).  With NBONDS (k = 54): only the first NBONDS bond
+      steps of the first forward pass.
 
   python tests/golden/make_golden.py rdm CFG D [NSAMPLE]
       rdm_cfgC_DD.npz - gamma and Gamma (Eq. 9-10, readings S2 / S20) of random_mps(seed = 900 + CFG,
@@ -88,21 +89,31 @@ def golden_heff(cid, D, bonds):
     print(out["note"], flush=True)
 
 
-def golden_sweep(cid, D, nsweeps, Dinit):
+def golden_sweep(cid, D, nsweeps, Dinit, nbonds=0):
+    """nbonds > 0 (large k, where a whole oracle sweep takes many hours): only the first nbonds bond steps of the forward
+    pass of the first sweep, in the sweep's own order (SweepEngine._optimise, the step sweep() itself calls); they do not
+    depend on the later ones."""
     cfg = make_config(cid)
     k, n = cfg["k"], cfg["n_elec"]
     mps = random_mps(k, n, cfg["two_sz"], Dinit, seed=cfg["seed"] + 1000, gauge="R")
     t0 = time.time()
     eng = odmrg.SweepEngine(cfg["h"], cfg["eri"], mps, davidson_tol=1e-10)
+    print("right environments built, %.0f s" % (time.time() - t0), flush=True)
     sweeps = []
-    for s in range(nsweeps):
+    if nbonds:
+        recs = []
+        for i in range(nbonds):
+            recs.append(eng._optimise(i, D, "fwd"))
+            print("config %d D=%d bond %d: E = %.12f, %d matvecs (%.0f s)" % (cid, D, i, recs[-1]["energy"], recs[-1]["n_matvec"], time.time() - t0), flush=True)
+        sweeps.append(dict(energy_last=None, energy_min=None, bonds=recs))
+    for s in range(0 if nbonds else nsweeps):
         r = eng.sweep(D)
         sweeps.append(r)
         print("config %d D=%d sweep %d: E_last = %.12f (%.0f s)" % (cid, D, s, r["energy_last"], time.time() - t0), flush=True)
-    note = ("written by `python tests/golden/make_golden.py sweep %d %d %d %d` from oracle.dmrg.SweepEngine "
-            "(Davidson tol 1e-10); oracle time %.0f s on %d host cores" % (cid, D, nsweeps, Dinit, time.time() - t0, os.cpu_count()))
+    note = ("written by `python tests/golden/make_golden.py sweep %d %d %d %d%s` from oracle.dmrg.SweepEngine "
+            "(Davidson tol 1e-10); oracle time %.0f s on %d host cores" % (cid, D, nsweeps, Dinit, " %d" % nbonds if nbonds else "", time.time() - t0, os.cpu_count()))
     with open(os.path.join(HERE, "sweep_cfg%d_D%d.json" % (cid, D)), "w") as f:
-        json.dump(dict(note=note, config=cid, D=D, Dinit=Dinit, mps_seed=cfg["seed"] + 1000, davidson_tol=1e-10,
+        json.dump(dict(note=note, config=cid, D=D, Dinit=Dinit, mps_seed=cfg["seed"] + 1000, davidson_tol=1e-10, partial_bonds=nbonds,
                        sweeps=[dict(energy_last=r["energy_last"], energy_min=r["energy_min"],
                                     bonds=[dict(bond=b["bond"], dir=b["dir"], energy=b["energy"], kept=b["kept"],
                                                 nsectors=b["nsectors"], trunc_err=b["trunc_err"], nnz=b["nnz"],
@@ -149,7 +160,7 @@ def main():
     elif what == "heff":
         golden_heff(a[0], a[1], a[2:])
     elif what == "sweep":
-        golden_sweep(a[0], a[1], a[2], a[3] if len(a) > 3 else a[1])
+        golden_sweep(a[0], a[1], a[2], a[3] if len(a) > 3 else a[1], a[4] if len(a) > 4 else 0)
     elif what == "rdm":
         golden_rdm(a[0], a[1], a[2] if len(a) > 2 else 0)
     else:

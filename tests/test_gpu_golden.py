@@ -76,9 +76,12 @@ def test_sweep_vs_golden(lib, name):
         lib.dmrg_mps_import(ctx, mps_to_blob_arrays(mps), k, n, s2)
         for s, gs in enumerate(gold["sweeps"]):
             r = lib.dmrg_sweep(ctx, D, k)
-            assert abs(r["energy_last"] - gs["energy_last"]) <= 1e-8
-            assert abs(r["energy_min"] - gs["energy_min"]) <= 1e-8
-            assert len(r["bonds"]) == len(gs["bonds"])
+            if gold.get("partial_bonds"):                        # k = 54: the oracle did the first bond steps of the forward pass only
+                assert len(gs["bonds"]) == gold["partial_bonds"] < len(r["bonds"])
+            else:
+                assert abs(r["energy_last"] - gs["energy_last"]) <= 1e-8
+                assert abs(r["energy_min"] - gs["energy_min"]) <= 1e-8
+                assert len(r["bonds"]) == len(gs["bonds"])
             for rg, ro in zip(r["bonds"], gs["bonds"]):
                 assert rg["bond"] == ro["bond"] and rg["forward"] == (1 if ro["dir"] == "fwd" else 0)
                 assert abs(rg["energy"] - ro["energy"]) <= 1e-8, (s, ro["bond"], ro["dir"])
