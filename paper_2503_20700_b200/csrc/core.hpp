@@ -292,6 +292,7 @@ struct Engine {
     // checkpoints are recomputed when a pass enters that segment; checkpoints optionally spilled to pinned host memory
     int env_stride = 1, env_stride2 = 1;
     bool env_spill = false;
+    int64_t ws_cap = 0;                           // doubles: cap of a T buffer chosen by the policy when the stack is checkpointed (0: none)
     HostPool host_pool;
     cudaStream_t copy_stream = nullptr;
     std::vector<Block*> pending_spills;

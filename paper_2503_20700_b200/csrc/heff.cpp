@@ -117,7 +117,7 @@ int64_t Engine::t_capacity() const {
     size_t free_b = 0, total_b = 0;
     if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) return (int64_t)1 << 27;
     int64_t cap = (int64_t)(free_b / 8) / 4;                   // a quarter of what is free ...
-    const int64_t hi = (int64_t)3 << 30;                       // ... at most 24 GiB
+    const int64_t hi = ws_cap > 0 ? ws_cap : (int64_t)3 << 30; // ... at most 24 GiB (6 GiB while the environment stack is checkpointed)
     const int64_t lo = (int64_t)1 << 24;
     return std::max(lo, std::min(cap, hi));
 }

@@ -490,49 +490,79 @@ void Engine::plan_env_policy(int D) {
     env_est_total = (int64_t)total; env_est_max = (int64_t)bmax;
     size_t free_b = 0, total_b = 0;
     cuda_check(cudaMemGetInfo(&free_b, &total_b), "cudaMemGetInfo");
-    // what is free now also has to hold the intermediates of H_eff psi and of the blocking step, the Davidson subspace
-    // and the block being grown: the stack gets 55 % of it unless the caller fixes a budget
-    const double budget = opt.hbm_budget_bytes > 0 ? (double)opt.hbm_budget_bytes : 0.55 * ((double)free_b + (double)g_device_bytes_env(*this));
+    // what is free now also has to hold the intermediates of H_eff psi and of the blocking step (two T buffers, capped at
+    // 6 GiB each once the stack is checkpointed), the Davidson subspace and allocator slack
+    const double avail = (double)free_b + (double)g_device_bytes_env(*this);
+    const double budget = opt.hbm_budget_bytes > 0 ? (double)opt.hbm_budget_bytes : std::max(0.55 * avail, 0.8 * avail - 20.0 * (double)(1ull << 30));
     const double host_budget = opt.host_budget_bytes > 0 ? (double)opt.host_budget_bytes : 64.0 * (double)(1ull << 30);
     env_spill = false;
+    env_stride = 1;
     env_stride2 = 1;
+    ws_cap = 0;
     if (opt.env_stride > 0) { env_stride = opt.env_stride; env_stride2 = std::max(1, opt.env_stride2); env_spill = opt.host_spill != 0; return; }
-    if (total <= budget) { env_stride = 1; return; }
-    if (opt.host_spill) {
-        // checkpoints on the host, the segment being consumed (stride blocks) plus the block being produced on the device
-        int s = 1;
-        while (s < k && total / s > host_budget) ++s;
-        env_stride2 = 1;
-        if ((s + 1) * bmax > budget) {
-            // a whole segment does not fit: second checkpoint level inside the segment (s / s2 kept blocks + s2 of the
-            // current sub-segment + the block being produced and the restored checkpoint)
-            int best2 = 0;
-            double need2 = 0.0;
-            for (int q = 2; q < s; ++q) {
-                const double need = ((s + q - 1) / q + q + 2) * bmax;
-                if (!best2 || need < need2) { best2 = q; need2 = need; }
+    if (total <= budget) return;
+    // Peak device bytes of the environment blocks over a whole sweep for checkpoint spacing s, second-level spacing q
+    // (1 = keep the whole segment) and checkpoints on the host or not: the resident sets of need_left / need_right /
+    // retire_* replayed on the per-bond estimates.
+    auto simulate = [&](int sp, int q, bool spill, double& host) {
+        auto ck = [&](int b) { return b == 0 || b == k || b % sp == 0; };
+        host = 0.0;
+        double cks = 0.0;
+        for (int c = 1; c < k; ++c) if (ck(c)) cks += est[c];
+        if (spill) host = 1.7 * cks;      // measured: the pinned pool peaks at 1.65-1.8 x one side's checkpoints (both sides at the turn-around, best-fit slack)
+        double peak = 0.0;
+        for (int i = 0; i <= k - 2; ++i) {
+            // forward pass: left side produces, right side is consumed
+            double left = est[i] + est[i + 1], right = 0.0;
+            if (spill) { if (i - 1 > 0 && ck(i - 1)) left += est[i - 1]; }             // spill copy still in flight
+            else for (int c = 1; c < i; ++c) if (ck(c)) left += est[c];
+            {
+                const int b = i + 2;
+                int c = b;
+                while (!ck(c)) ++c;
+                const int kb = (b / q + 1) * q;
+                for (int j = b; j <= c; ++j) if (j == c || j % q == 0 || j < kb) right += est[j];
+                if (!spill) for (int c2 = c + 1; c2 < k; ++c2) if (ck(c2)) right += est[c2];
             }
-            if (!best2 || need2 > budget) throw Error(-3, "environment stack: one segment between host checkpoints exceeds the device budget");
-            env_stride = s; env_stride2 = best2; env_spill = true;
-            return;
+            peak = std::max(peak, left + right);
+            // backward pass: right side produces, left side is consumed
+            right = est[i + 2] + est[i + 1];
+            left = 0.0;
+            if (spill) { if (i + 3 < k && ck(i + 3)) right += est[i + 3]; }
+            else for (int c = i + 3; c < k; ++c) if (ck(c)) right += est[c];
+            {
+                const int b = i;
+                int c = b;
+                while (!ck(c)) --c;
+                const int ka = b > 0 ? ((b - 1) / q) * q : 0;
+                for (int j = c; j <= b; ++j) if (j == c || j % q == 0 || j > ka) left += est[j];
+                if (!spill) for (int c2 = 1; c2 < c; ++c2) if (ck(c2)) left += est[c2];
+            }
+            peak = std::max(peak, left + right);
         }
-        // fewer, larger segments while they stay within half the budget (at most 8 blocks): pinning host memory for a
-        // checkpoint costs more than recomputing a block (measured, config 4 at D = 2048: stride 6 -> 319 s, stride 2 -> 346 s
-        // for the first sweep; later sweeps reuse the pinned pool)
-        while (s < 8 && s + 1 < k && (s + 2) * bmax <= 0.5 * budget) ++s;
-        env_stride = s; env_spill = true;
-        return;
-    }
-    int best = 0;
-    double best_need = 0.0;
-    for (int s = 1; s <= k; ++s) {
-        const double need = total / s + (s + 1) * bmax;
-        if (!best || need < best_need) { best = s; best_need = need; }
-    }
-    if (best_need > budget) throw Error(-3, "environment stack does not fit the device even with recomputation: set host_spill = 1");
-    int s = 1;
-    while (total / s + (s + 1) * bmax > budget) ++s;                  // smallest stride that fits: least recomputation
-    env_stride = s;
+        return peak;
+    };
+    // cheapest feasible setting: cost = fraction of blocks recomputed per pass (second level: again) + a small charge for
+    // the host round trips
+    int bs = 0, bq = 1;
+    bool bspill = false;
+    double bcost = 0.0, bpeak = 0.0;
+    for (int spill = 0; spill <= (opt.host_spill ? 1 : 0); ++spill)
+        for (int sp = 1; sp <= std::min(k, 24); ++sp)
+            for (int q = 1; q < std::max(2, sp); ++q) {
+                if (sp == 1 && !spill) continue;                      // everything resident: already ruled out above
+                double host = 0.0;
+                const double peak = simulate(sp, q, spill != 0, host);
+                if (peak > budget || host > host_budget) continue;
+                const double r1 = (double)(sp - 1) / sp;
+                const double cost = r1 + (q > 1 ? r1 * (q - 1) / q : 0.0) + (spill ? 0.3 / sp : 0.0);
+                if (!bs || cost < bcost - 1e-12 || (cost < bcost + 1e-12 && peak < bpeak)) { bs = sp; bq = q; bspill = spill != 0; bcost = cost; bpeak = peak; }
+            }
+    if (!bs)
+        throw Error(-3, opt.host_spill ? "environment stack does not fit the device and host budgets even with two checkpoint levels"
+                                       : "environment stack does not fit the device even with recomputation: set host_spill = 1");
+    env_stride = bs; env_stride2 = bq; env_spill = bspill;
+    if (opt.workspace_bytes == 0) ws_cap = (int64_t)6 << 27;          // 6 GiB of doubles per T buffer while memory is tight
 }
 
 void Engine::finish_spills() {

@@ -187,7 +187,9 @@ def test_config4_reduced_D_sweep_memory_path_and_rdm(lib):
             lib.dmrg_destroy(ctx)
     (ra, sa, g, G), (rb, sb, _, _) = out
     assert sa["env_stride"] == 1 and sa["host_spill"] == 0
-    assert sb["env_stride"] > 1 and sb["host_spill"] == 1 and sb["bytes_spilled"] > 0 and sb["seconds_regrow"] > 0
+    assert sb["env_stride"] > 1 and sb["seconds_regrow"] > 0           # the automatic policy had to checkpoint ...
+    assert sb["host_spill"] == 1 and sb["bytes_spilled"] > 0           # ... and, with these budgets, to spill
+    assert sb["peak_device_bytes"] < sa["peak_device_bytes"]
     assert [b["energy"] for b in ra["bonds"]] == [b["energy"] for b in rb["bonds"]]
     assert [b["kept"] for b in ra["bonds"]] == [b["kept"] for b in rb["bonds"]]
     assert abs(np.trace(g) - n) <= 1e-9
