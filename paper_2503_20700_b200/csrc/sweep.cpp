@@ -500,7 +500,8 @@ void Engine::plan_env_policy(int D) {
     env_stride2 = 1;
     ws_cap = 0;
     if (opt.env_stride > 0) { env_stride = opt.env_stride; env_stride2 = std::max(1, opt.env_stride2); env_spill = opt.host_spill != 0; return; }
-    if (total <= budget) return;
+    // everything resident only with headroom for the two full-size (24 GiB) T buffers of H_eff psi
+    if (total <= (opt.hbm_budget_bytes > 0 ? budget : budget - 24.0 * (double)(1ull << 30))) return;
     // Peak device bytes of the environment blocks over a whole sweep for checkpoint spacing s, second-level spacing q
     // (1 = keep the whole segment) and checkpoints on the host or not: the resident sets of need_left / need_right /
     // retire_* replayed on the per-bond estimates.
