@@ -25,7 +25,7 @@ def test_golden_files_present():
     """configs 4 and 5 must have an H_eff golden, configs 2 and 3 a sweep and an RDM golden."""
     for c in (4, 5):
         assert _files("heff_cfg%d_D*.npz" % c)
-    assert _files("rdm_cfg4_D*.npz")                              # k = 54: the half-chain RDM pass vs the oracle's pass
+    assert _files("rdm_cfg4_D*.npz") and _files("rdm_cfg5_D*.npz")   # k = 54, 82: the half-chain RDM pass vs the oracle's pass
     for c in (2, 3, 6):                                           # 6: the open-shell second workload (2Sz = 5, odd N)
         assert _files("sweep_cfg%d_D*.json" % c) and _files("rdm_cfg%d_D*.npz" % c)
 
