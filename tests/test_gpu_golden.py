@@ -28,6 +28,7 @@ def test_golden_files_present():
     assert _files("rdm_cfg4_D*.npz") and _files("rdm_cfg5_D*.npz")   # k = 54, 82: the half-chain RDM pass vs the oracle's pass
     for c in (2, 3, 6):                                           # 6: the open-shell second workload (2Sz = 5, odd N)
         assert _files("sweep_cfg%d_D*.json" % c) and _files("rdm_cfg%d_D*.npz" % c)
+    assert _files("sweep_cfg4_D*.json") and _files("sweep_cfg5_D*.json")   # k = 54, 82: the first bond steps of a sweep
 
 
 @pytest.mark.parametrize("name", _files("heff_cfg*_D*.npz"))
