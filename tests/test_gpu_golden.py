@@ -29,6 +29,7 @@ def test_golden_files_present():
     for c in (2, 3, 6):                                           # 6: the open-shell second workload (2Sz = 5, odd N)
         assert _files("sweep_cfg%d_D*.json" % c) and _files("rdm_cfg%d_D*.npz" % c)
     assert _files("sweep_cfg4_D*.json") and _files("sweep_cfg5_D*.json")   # k = 54, 82: the first bond steps of a sweep
+    assert _files("sweep_cfg1_D*.json")                           # config 1 at D = 64: all 4 sweeps
 
 
 @pytest.mark.parametrize("name", _files("heff_cfg*_D*.npz"))
@@ -88,6 +89,9 @@ def test_sweep_vs_golden(lib, name):
                 assert abs(rg["energy"] - ro["energy"]) <= 1e-8, (s, ro["bond"], ro["dir"])
                 assert rg["kept"] == ro["kept"] and rg["nsectors"] == ro["nsectors"] and rg["nnz"] == ro["nnz"]
                 assert abs(rg["trunc_err"] - ro["trunc_err"]) <= 1e-9
+        if gold["config"] == 1:                                  # variational: never below the oracle's brute-force FCI energy
+            fci = [float(l.split()[1]) for l in open(os.path.join(GOLD, "config1_fci.txt")) if l.startswith("e_total_fci")][0]
+            assert r["energy_last"] + cfg["e_core"] >= fci - 1e-8
     finally:
         lib.dmrg_destroy(ctx)
 

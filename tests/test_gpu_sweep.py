@@ -58,16 +58,8 @@ def test_untruncated_sweep_reaches_fci(lib):
         lib.dmrg_destroy(ctx)
 
 
-def test_sweep_config1_naphthalene_D64(lib):
-    """BASELINE config 1 at D=64, 4 sweeps: per-sweep energies GPU vs oracle (reading S11: D=64 is truncated)."""
-    cfg = make_config(1)
-    k, n = cfg["k"], cfg["n_elec"]
-    res = _run_both(lib, cfg["h"], cfg["eri"], k, n, 0, 64, cfg["sweeps"], seed=cfg["seed"] + 1000)
-    for (g, o) in res:
-        assert abs(g["energy_last"] - o["energy_last"]) <= TOL_E
-        assert abs(g["energy_min"] - o["energy_min"]) <= TOL_E
-    # variational: never below the FCI energy quoted in tests/golden (computed by the oracle's brute force)
-    assert res[-1][0]["energy_last"] + cfg["e_core"] >= -0.8822829988 - 1e-8
+# BASELINE config 1 at D = 64, 4 sweeps (reading S11: D = 64 is truncated): per-bond parity with the oracle is in
+# tests/test_gpu_golden.py::test_sweep_vs_golden[sweep_cfg1_D64.json] (stored oracle result; the live oracle took 2 min here).
 
 
 def _golden():
